@@ -1,3 +1,283 @@
 """B200-native SHARP projection loop (arXiv 1602.01448): ctypes binding over the C-ABI library
-`libsharp_b200.so` (include/sharp_b200.h).  The library is loaded on first use and the load fails loudly if
-it has not been built (`python -c "import __graft_entry__ as g; g.build()"`); there is no CPU fallback."""
+`libsharp_b200.so` (include/sharp_b200.h).
+
+The binding only marshals arguments: every step of the method runs in the library's CUDA kernels.  PyTorch is
+used for device memory and streams, nothing else.  The library is loaded on first use and the load fails loudly
+if it has not been built (`python -c "import __graft_entry__ as g; g.build()"`); there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsharp_b200.so")
+HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "sharp_b200.h")
+
+SHARP_OK, SHARP_EINVAL, SHARP_ESTATE, SHARP_ENOMEM, SHARP_ECUDA = 0, -1, -2, -3, -4
+TILE = 32
+
+_vp, _i, _f, _sz, _ll = C.c_void_p, C.c_int, C.c_float, C.c_size_t, C.c_longlong
+_SIGNATURES = {
+    "sharp_plan": (_i, [C.POINTER(_vp), _i, _i, _vp, _i, _i]),
+    "sharp_destroy": (None, [_vp]),
+    "sharp_last_error": (C.c_char_p, [_vp]),
+    "sharp_workspace_bytes": (_sz, [_vp]),
+    "sharp_bind": (_i, [_vp, _vp, _sz, _vp]),
+    "sharp_set_intensities": (_i, [_vp, _vp]),
+    "sharp_set_probe": (_i, [_vp, _vp]),
+    "sharp_set_object": (_i, [_vp, _vp]),
+    "sharp_set_frames": (_i, [_vp, _vp]),
+    "sharp_set_probe_refine": (_i, [_vp, _i]),
+    "sharp_iterate": (_i, [_vp, _i, _f]),
+    "sharp_get_object": (_i, [_vp, _vp]),
+    "sharp_get_probe": (_i, [_vp, _vp]),
+    "sharp_get_frames": (_i, [_vp, _vp]),
+    "sharp_get_amplitudes": (_i, [_vp, _vp]),
+    "sharp_errors": (_i, [_vp, C.POINTER(_f)]),
+    "sharp_sync": (_i, [_vp]),
+    "sharp_launch_count": (_ll, [_vp]),
+    "sharp_tile_grid": (_i, [_vp, C.POINTER(_i), C.POINTER(_i)]),
+    "sharp_tile_lists": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
+    "sharp_cover_counts": (_i, [_vp, _vp]),
+    "sharp_frame_index": (_i, [_vp, _vp]),
+    "sharp_op_split": (_i, [_vp, _vp, _vp]),
+    "sharp_op_overlap": (_i, [_vp, _vp, _vp]),
+    "sharp_op_pa": (_i, [_vp, _vp, _vp]),
+    "sharp_op_fft2": (_i, [_vp, _vp, _vp, _i]),
+    "sharp_op_probe": (_i, [_vp, _vp, _vp, _vp]),
+    "sharp_reconstruct_host": (_i, [_vp, _vp, _vp, _i, _f, _vp, _vp, C.POINTER(_f)]),
+}
+
+_lib = None
+
+
+class SharpError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"sharp_b200 error {code}: {text}")
+        self.code = code
+
+
+def load_library():
+    """dlopen libsharp_b200.so and bind every symbol include/sharp_b200.h declares.  Raises if the library is
+    missing or a symbol is not exported (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} has not been built; run `python -c 'import __graft_entry__ as g; g.build()'`")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(lib, name)          # AttributeError if the symbol is missing
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def exported_symbols():
+    return sorted(_SIGNATURES)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(None)
+
+
+class Reconstruction:
+    """One plan bound to one torch device/stream.  Methods have the names of the C calls without the prefix.
+    Array arguments may be numpy arrays or torch tensors; they are moved to the device as float32 / complex64."""
+
+    def __init__(self, m, positions, obj_shape, device="cuda:0", stream=None):
+        import torch
+        self._torch = torch
+        self.lib = load_library()
+        self.m = int(m)
+        pos = np.ascontiguousarray(positions, dtype=np.int32)
+        if pos.ndim != 2 or pos.shape[1] != 2:
+            raise ValueError("positions must be (K, 2) int32 (row, col)")
+        self.K = int(pos.shape[0])
+        self.shape = (int(obj_shape[0]), int(obj_shape[1]))
+        self._plan = C.c_void_p(None)
+        rc = self.lib.sharp_plan(C.byref(self._plan), self.m, self.K, pos.ctypes.data_as(C.c_void_p), *self.shape)
+        if rc != SHARP_OK:
+            raise SharpError(rc, self.lib.sharp_last_error(None).decode())
+        self.device = torch.device(device) if device is not None else None
+        self._ws = None
+        if self.device is not None:
+            if not torch.cuda.is_available():
+                raise SharpError(SHARP_ECUDA, "no CUDA device: this library has no CPU path")
+            nbytes = int(self.lib.sharp_workspace_bytes(self._plan))
+            with torch.cuda.device(self.device):
+                self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+                self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+                off = (-self._ws.data_ptr()) % 256
+                self._check(self.lib.sharp_bind(self._plan, C.c_void_p(self._ws.data_ptr() + off), nbytes,
+                                                C.c_void_p(self._stream.cuda_stream)))
+
+    # -- plumbing ----------------------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != SHARP_OK:
+            raise SharpError(rc, self.lib.sharp_last_error(self._plan).decode())
+
+    def _dev(self, x, dtype):
+        torch = self._torch
+        if x is None:
+            return None
+        if not torch.is_tensor(x):
+            x = torch.from_numpy(np.ascontiguousarray(x))
+        with torch.cuda.stream(self._stream):
+            return x.to(device=self.device, dtype=dtype, non_blocking=False).contiguous()
+
+    def _new(self, shape, dtype):
+        with self._torch.cuda.stream(self._stream):
+            return self._torch.empty(shape, dtype=dtype, device=self.device)
+
+    def close(self):
+        if getattr(self, "_plan", None) is not None and self._plan.value:
+            if self._ws is not None:
+                self._torch.cuda.synchronize(self.device)
+            self.lib.sharp_destroy(self._plan)
+            self._plan = C.c_void_p(None)
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C calls ---------------------------------------------------------------------------------------------
+    def workspace_bytes(self):
+        return int(self.lib.sharp_workspace_bytes(self._plan))
+
+    def set_intensities(self, I):
+        t = self._dev(I, self._torch.float32)
+        assert t.numel() == self.K * self.m * self.m
+        self._check(self.lib.sharp_set_intensities(self._plan, _ptr(t)))
+        self._keep_I = t    # alive until the stream work is done
+
+    def set_probe(self, w):
+        t = self._dev(w, self._torch.complex64)
+        assert t.numel() == self.m * self.m
+        self._check(self.lib.sharp_set_probe(self._plan, _ptr(t)))
+        self._keep_w = t
+
+    def set_object(self, psi=None):
+        t = self._dev(psi, self._torch.complex64)
+        assert t is None or t.numel() == self.shape[0] * self.shape[1]
+        self._check(self.lib.sharp_set_object(self._plan, _ptr(t)))
+        self._keep_psi = t
+
+    def set_frames(self, z):
+        t = self._dev(z, self._torch.complex64)
+        assert t.numel() == self.K * self.m * self.m
+        self._check(self.lib.sharp_set_frames(self._plan, _ptr(t)))
+        self._keep_z = t
+
+    def set_probe_refine(self, every):
+        self._check(self.lib.sharp_set_probe_refine(self._plan, int(every)))
+
+    def iterate(self, n, beta):
+        self._check(self.lib.sharp_iterate(self._plan, int(n), float(beta)))
+
+    def get_object(self):
+        out = self._new(self.shape, self._torch.complex64)
+        self._check(self.lib.sharp_get_object(self._plan, _ptr(out)))
+        return out
+
+    def get_probe(self):
+        out = self._new((self.m, self.m), self._torch.complex64)
+        self._check(self.lib.sharp_get_probe(self._plan, _ptr(out)))
+        return out
+
+    def get_frames(self):
+        out = self._new((self.K, self.m, self.m), self._torch.complex64)
+        self._check(self.lib.sharp_get_frames(self._plan, _ptr(out)))
+        return out
+
+    def get_amplitudes(self):
+        out = self._new((self.K, self.m, self.m), self._torch.float32)
+        self._check(self.lib.sharp_get_amplitudes(self._plan, _ptr(out)))
+        return out
+
+    def errors(self):
+        out = (C.c_float * 3)()
+        self._check(self.lib.sharp_errors(self._plan, out))
+        return np.array([out[0], out[1], out[2]], dtype=np.float64)
+
+    def sync(self):
+        self._check(self.lib.sharp_sync(self._plan))
+
+    def launch_count(self):
+        return int(self.lib.sharp_launch_count(self._plan))
+
+    # integer artefacts
+    def tile_grid(self):
+        a, b = C.c_int(0), C.c_int(0)
+        self._check(self.lib.sharp_tile_grid(self._plan, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def tile_lists(self):
+        tr, tc = self.tile_grid()
+        p, f = C.c_void_p(None), C.c_void_p(None)
+        self._check(self.lib.sharp_tile_lists(self._plan, C.byref(p), C.byref(f)))
+        ptr = np.ctypeslib.as_array(C.cast(p, C.POINTER(C.c_int32)), shape=(tr * tc + 1,)).copy()
+        n = int(ptr[-1])
+        frames = np.ctypeslib.as_array(C.cast(f, C.POINTER(C.c_int32)), shape=(n,)).copy() if n else np.zeros(0, np.int32)
+        return ptr, frames
+
+    def cover_counts(self):
+        out = np.empty(self.shape, dtype=np.int32)
+        self._check(self.lib.sharp_cover_counts(self._plan, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def frame_index(self):
+        out = self._new((self.K, self.m, self.m), self._torch.int64)
+        self._check(self.lib.sharp_frame_index(self._plan, _ptr(out)))
+        return out
+
+    # single operators (test hooks)
+    def op_split(self, psi):
+        t = self._dev(psi, self._torch.complex64)
+        out = self._new((self.K, self.m, self.m), self._torch.complex64)
+        self._check(self.lib.sharp_op_split(self._plan, _ptr(t), _ptr(out)))
+        return out
+
+    def op_overlap(self, f):
+        t = self._dev(f, self._torch.complex64)
+        out = self._new(self.shape, self._torch.complex64)
+        self._check(self.lib.sharp_op_overlap(self._plan, _ptr(t), _ptr(out)))
+        return out
+
+    def op_pa(self, f):
+        t = self._dev(f, self._torch.complex64)
+        out = self._new((self.K, self.m, self.m), self._torch.complex64)
+        self._check(self.lib.sharp_op_pa(self._plan, _ptr(t), _ptr(out)))
+        return out
+
+    def op_fft2(self, f, sign=-1):
+        t = self._dev(f, self._torch.complex64)
+        out = self._new((self.K, self.m, self.m), self._torch.complex64)
+        self._check(self.lib.sharp_op_fft2(self._plan, _ptr(t), _ptr(out), int(sign)))
+        return out
+
+    def op_probe(self, psi, z):
+        tp = self._dev(psi, self._torch.complex64)
+        tz = self._dev(z, self._torch.complex64)
+        out = self._new((self.m, self.m), self._torch.complex64)
+        self._check(self.lib.sharp_op_probe(self._plan, _ptr(tp), _ptr(tz), _ptr(out)))
+        return out
+
+    def reconstruct_host(self, I_host, w_host, n, beta, want_eps=True):
+        """HOST buffers in, HOST buffers out (torch CPU tensors, ideally pinned).  Returns (psi, w, eps)."""
+        torch = self._torch
+        assert I_host.dtype == torch.float32 and I_host.is_contiguous() and not I_host.is_cuda
+        assert w_host.dtype == torch.complex64 and w_host.is_contiguous() and not w_host.is_cuda
+        if getattr(self, "_host_out", None) is None:
+            self._host_out = (torch.empty(self.shape, dtype=torch.complex64).pin_memory(),
+                              torch.empty((self.m, self.m), dtype=torch.complex64).pin_memory())
+        psi, w = self._host_out
+        eps = (C.c_float * 3)()
+        self._check(self.lib.sharp_reconstruct_host(self._plan, _ptr(I_host), _ptr(w_host), int(n), float(beta),
+                                                    _ptr(psi), _ptr(w), eps if want_eps else None))
+        return psi, w, np.array([eps[0], eps[1], eps[2]], dtype=np.float64)

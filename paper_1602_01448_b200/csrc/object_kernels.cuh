@@ -1,0 +1,308 @@
+// object_kernels.cuh -- everything that is not the fused FFT kernel: split (a1), the deterministic gather-form
+// overlap with its object-space epilogues (a5 + the object half of a6), the illumination refinement (a7), the
+// amplitude preparation (a0) and small helpers.
+#pragma once
+#include "frame_kernel.cuh"
+
+namespace sharp {
+
+constexpr int TILE = 32;  // == SHARP_TILE
+
+// ---------------------------------------------------------------------------------------------------------
+// a1 split:  z_i(r) = w(r) psi(r + x_i).  One thread per two consecutive frame pixels of a
+// row: 128-bit loads of w and stores of z; psi is only 8-byte aligned (x_i.col is arbitrary) so it is read as
+// two 64-bit loads.  psi == NULL means the flat object 1 + 0i (reading G8).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_split(int m, int K, const int *pos, int nc, const float2 *psi,
+                                                const float2 *w, float2 *z)
+{
+    const size_t half = (size_t)m / 2;
+    const size_t per_frame = (size_t)m * half;
+    const size_t total = (size_t)K * per_frame;
+    for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(g / per_frame);
+        const size_t rem = g - (size_t)i * per_frame;
+        const int r = (int)(rem / half), c = 2 * (int)(rem % half);
+        const float4 w2 = __ldg(reinterpret_cast<const float4 *>(w + (size_t)r * m + c));
+        float2 p0 = make_float2(1.f, 0.f), p1 = p0;
+        if (psi != nullptr) {
+            const float2 *pp = psi + (size_t)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + c);
+            p0 = __ldg(pp);
+            p1 = __ldg(pp + 1);
+        }
+        const float2 z0 = cmul(make_float2(w2.x, w2.y), p0), z1 = cmul(make_float2(w2.z, w2.w), p1);
+        __stcs(reinterpret_cast<float4 *>(z + ((size_t)i * m + r) * m + c), make_float4(z0.x, z0.y, z1.x, z1.y));
+    }
+}
+
+// z = c + w_form . T psi_v  (materialise the frames kept in factored form; sharp_get_frames)
+__global__ void __launch_bounds__(256) k_materialize(int m, int K, const int *pos, int nc, const float2 *c,
+                                                      const float2 *psi_v, const float2 *w, float2 *z)
+{
+    const size_t per_frame = (size_t)m * m;
+    const size_t total = (size_t)K * per_frame;
+    for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(g / per_frame);
+        const size_t rem = g - (size_t)i * per_frame;
+        const int r = (int)(rem / m), col = (int)(rem % m);
+        float2 v = __ldcs(c + g);
+        if (psi_v != nullptr)
+            v = cadd(v, cmul(__ldg(w + rem), __ldg(psi_v + (size_t)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + col))));
+        z[g] = v;
+    }
+}
+
+// linear object index of frame pixel (i, r, c), with the same expression the kernels above use (O10 (i))
+__global__ void __launch_bounds__(256) k_frame_index(int m, int K, const int *pos, int nc, long long *idx)
+{
+    const size_t per_frame = (size_t)m * m;
+    const size_t total = (size_t)K * per_frame;
+    for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(g / per_frame);
+        const size_t rem = g - (size_t)i * per_frame;
+        const int r = (int)(rem / m), col = (int)(rem % m);
+        idx[g] = (long long)((size_t)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + col));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// a0 amplitudes:  a = sqrt(max(I, 0))  (reading G14), stored as a/m in the FFT's position space:
+//     a_int[i][q][p] = a[i][freq(q)][freq(p)] / m,   freq(x) = x / RB + RA (x % RB).
+// Also per-block partial sums of max(I,0) in double (||a||^2, reading G12); k_scalars finishes them in a fixed
+// order.  natural != 0 is the inverse map (a_int -> a, for sharp_get_amplitudes).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_amplitudes(int m, int RA, int K, const float *I, float *a_int,
+                                                     double *partials)
+{
+    const int RB = m / RA;
+    const size_t per_frame = (size_t)m * m;
+    const size_t total = (size_t)K * per_frame;
+    const float inv_m = 1.0f / (float)m;
+    double acc = 0.0;
+    for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = g / per_frame;
+        const size_t rem = g - i * per_frame;
+        const int q = (int)(rem / m), p = (int)(rem % m);
+        const int u = q / RB + RA * (q % RB), v = p / RB + RA * (p % RB);
+        const float val = fmaxf(__ldg(I + i * per_frame + (size_t)u * m + v), 0.0f);
+        acc += (double)val;
+        a_int[g] = sqrtf(val) * inv_m;
+    }
+    __shared__ double red[256];
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int off = 128; off > 0; off >>= 1) {
+        if ((int)threadIdx.x < off) red[threadIdx.x] += red[threadIdx.x + off];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partials[blockIdx.x] = red[0];
+}
+
+__global__ void k_amplitudes_natural(int m, int RA, int K, const float *a_int, float *a)
+{
+    const int RB = m / RA;
+    const size_t per_frame = (size_t)m * m;
+    const size_t total = (size_t)K * per_frame;
+    for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = g / per_frame;
+        const size_t rem = g - i * per_frame;
+        const int q = (int)(rem / m), p = (int)(rem % m);
+        const int u = q / RB + RA * (q % RB), v = p / RB + RA * (p % RB);
+        a[i * per_frame + (size_t)u * m + v] = a_int[g] * (float)m;
+    }
+}
+
+// A2 = sum of the partials in index order; thr2 = (m thr)^2 = tau^2 A2 / K  with thr = tau a_rms (reading G4).
+__global__ void k_scalars(int nparts, const double *partials, int K, double tau, DevScalars *sc)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double s = 0.0;
+        for (int j = 0; j < nparts; ++j) s += partials[j];
+        sc->A2 = s;
+        sc->thr2 = (float)(tau * tau * s / (double)K);
+        sc->pad = 0.f;
+    }
+}
+
+// sums gridDim-many triples in index order into out[3] (eps numerators, doubles)
+__global__ void k_sum_triples(int n, const double *partials, double *out)
+{
+    if (threadIdx.x < 3 && blockIdx.x == 0) {
+        double s = 0.0;
+        for (int j = 0; j < n; ++j) s += partials[3 * j + threadIdx.x];
+        out[threadIdx.x] = s;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// a5 overlap, gather form (PAPER.md:153-155 Eq. 9; :224 "the image is divided into blocks ... each block
+// determines which frames contribute").  One CTA per TILE x TILE object tile; the tile's CSR list gives the
+// frames that touch it, in ascending frame index, so every pixel's sum runs in ascending i with no atomics
+// (reading G17).  256 threads, each owning one column and four rows (ty, ty+8, ty+16, ty+24) of the tile.
+//
+//   num(p)   = sum_i conj(w_a(p - x_i)) f_i(p - x_i)
+//   cross(p) = sum_i conj(w_a(p - x_i)) w_b(p - x_i)            (OV_REGATHER only)
+//   den(p)   = sum_i |w_a(p - x_i)|^2                            (OV_DEN only; otherwise read from the den array)
+// Epilogues:
+//   OV_DEN       den[p] = sum |w_a|^2
+//   OV_L         out[p] = num/den, 0 where den == 0 (reading G5)
+//   OV_ITER      psi_c = num/den; psi_y = (psi_c - beta psi_z)/(1 - 2 beta); psi_v[p] = beta (2 psi_y - psi_z);
+//                psi_z[p] = psi_y                                (object half of RAAR)
+//   OV_REGATHER  psi_z[p] = (num + psi_v[p] cross)/den           (L_{w_a}(c + w_b . T psi_v) after w changed)
+// ---------------------------------------------------------------------------------------------------------
+enum OverlapMode : int { OV_DEN = 0, OV_L = 1, OV_ITER = 2, OV_REGATHER = 3 };
+
+struct OverlapArgs {
+    int m, nr, nc, tiles_c;
+    const int *pos;
+    const int *tile_ptr;
+    const int *tile_frames;
+    const float2 *f;        // K m m
+    const float2 *w_a;      // m m
+    const float2 *w_b;      // m m (REGATHER)
+    float *den;             // object-sized
+    float2 *out;            // OV_L
+    float2 *psi_z;          // ITER in/out, REGATHER out
+    const float2 *psi_v_in; // REGATHER
+    float2 *psi_v_out;      // ITER
+    float beta;
+};
+
+template <int MODE>
+__global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
+{
+    const int tile = blockIdx.x;
+    const int tr = tile / A.tiles_c, tc = tile % A.tiles_c;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int pc = tc * TILE + tx;
+    const int pr0 = tr * TILE + ty;
+    const int m = A.m;
+    const int beg = A.tile_ptr[tile], end = A.tile_ptr[tile + 1];
+
+    float2 num[4], cr[4];
+    float dn[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        num[k] = make_float2(0.f, 0.f);
+        cr[k] = make_float2(0.f, 0.f);
+        dn[k] = 0.f;
+    }
+
+    for (int e = beg; e < end; ++e) {
+        const int fi = __ldg(A.tile_frames + e);
+        const int xr = __ldg(A.pos + 2 * fi), xc = __ldg(A.pos + 2 * fi + 1);
+        const int cc = pc - xc;
+        if ((unsigned)cc >= (unsigned)m) continue;
+        const float2 *fb = (MODE == OV_DEN) ? nullptr : A.f + (size_t)fi * m * m;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int rr = pr0 + 8 * k - xr;
+            if ((unsigned)rr < (unsigned)m) {
+                const int off = rr * m + cc;
+                const float2 wa = __ldg(A.w_a + off);
+                if constexpr (MODE == OV_DEN) {
+                    dn[k] += wa.x * wa.x + wa.y * wa.y;
+                } else {
+                    const float2 fv = __ldcs(fb + off);
+                    // conj(wa) * fv
+                    num[k].x += wa.x * fv.x + wa.y * fv.y;
+                    num[k].y += wa.x * fv.y - wa.y * fv.x;
+                    if constexpr (MODE == OV_REGATHER) {
+                        const float2 wb = __ldg(A.w_b + off);
+                        cr[k].x += wa.x * wb.x + wa.y * wb.y;
+                        cr[k].y += wa.x * wb.y - wa.y * wb.x;
+                    }
+                }
+            }
+        }
+    }
+
+    if (pc >= A.nc) return;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int pr = pr0 + 8 * k;
+        if (pr >= A.nr) continue;
+        const size_t p = (size_t)pr * A.nc + pc;
+        if constexpr (MODE == OV_DEN) {
+            A.den[p] = dn[k];
+        } else {
+            const float d = A.den[p];
+            const bool lit = d > 0.f;
+            if constexpr (MODE == OV_L) {
+                A.out[p] = lit ? make_float2(num[k].x / d, num[k].y / d) : make_float2(0.f, 0.f);
+            } else if constexpr (MODE == OV_ITER) {
+                float2 py = make_float2(0.f, 0.f), pv = py;
+                if (lit) {
+                    const float2 pz = A.psi_z[p];
+                    const float inv = 1.0f / (1.0f - 2.0f * A.beta);
+                    py.x = (num[k].x / d - A.beta * pz.x) * inv;
+                    py.y = (num[k].y / d - A.beta * pz.y) * inv;
+                    pv.x = A.beta * (2.0f * py.x - pz.x);
+                    pv.y = A.beta * (2.0f * py.y - pz.y);
+                }
+                A.psi_z[p] = py;
+                A.psi_v_out[p] = pv;
+            } else {  // OV_REGATHER
+                float2 o = make_float2(0.f, 0.f);
+                if (lit) {
+                    float2 t = num[k];
+                    if (A.psi_v_in != nullptr) t = cadd(t, cmul(A.psi_v_in[p], cr[k]));
+                    o = make_float2(t.x / d, t.y / d);
+                }
+                A.psi_z[p] = o;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// a7 illumination refinement, Eq. (10) PAPER.md:157-159:
+//     w(r) <- sum_i conj(psi(r + x_i)) z_i(r) / sum_i |psi(r + x_i)|^2
+// with z_i = c_i + w_form . T psi_v formed on the fly.  Two stages, both in a fixed order: each CTA column sums
+// a chunk of consecutive frames (ascending i) per probe pixel; k_probe_final adds the chunks in ascending order
+// and divides; where the denominator is 0 the old value is kept.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_probe_partial(int m, int K, int chunk, const int *pos, int nc,
+                                                        const float2 *c, const float2 *psi_v, const float2 *w_form,
+                                                        const float2 *psi, float2 *pnum, float *pden)
+{
+    const int pix = blockIdx.x * blockDim.x + threadIdx.x;  // m*m is a multiple of 256
+    const int r = pix / m, col = pix % m;
+    const int i0 = blockIdx.y * chunk, i1 = min(K, i0 + chunk);
+    const float2 wf = __ldg(w_form + pix);
+    float2 num = make_float2(0.f, 0.f);
+    float den = 0.f;
+    for (int i = i0; i < i1; ++i) {
+        const size_t op = (size_t)(__ldg(pos + 2 * i) + r) * nc + (__ldg(pos + 2 * i + 1) + col);
+        const float2 ps = __ldg(psi + op);
+        float2 z = __ldcs(c + (size_t)i * m * m + pix);
+        if (psi_v != nullptr) z = cadd(z, cmul(wf, __ldg(psi_v + op)));
+        num.x += ps.x * z.x + ps.y * z.y;  // conj(ps) * z
+        num.y += ps.x * z.y - ps.y * z.x;
+        den += ps.x * ps.x + ps.y * ps.y;
+    }
+    pnum[(size_t)blockIdx.y * m * m + pix] = num;
+    pden[(size_t)blockIdx.y * m * m + pix] = den;
+}
+
+__global__ void __launch_bounds__(256) k_probe_final(int m, int nchunks, const float2 *pnum, const float *pden,
+                                                      const float2 *w_old, float2 *w_new)
+{
+    const int pix = blockIdx.x * blockDim.x + threadIdx.x;
+    float2 num = make_float2(0.f, 0.f);
+    float den = 0.f;
+    for (int j = 0; j < nchunks; ++j) {
+        const float2 a = pnum[(size_t)j * m * m + pix];
+        num.x += a.x;
+        num.y += a.y;
+        den += pden[(size_t)j * m * m + pix];
+    }
+    w_new[pix] = den > 0.f ? make_float2(num.x / den, num.y / den) : w_old[pix];
+}
+
+__global__ void k_fill_c64(size_t n, float2 *p, float2 v)
+{
+    for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < n; g += (size_t)gridDim.x * blockDim.x) p[g] = v;
+}
+
+}  // namespace sharp

@@ -1,0 +1,686 @@
+// sharp_b200.cu -- host side of the C ABI declared in include/sharp_b200.h: the plan (integer geometry, tile
+// lists, workspace layout), the iteration schedule and the kernel launches.  All arithmetic of the method runs in
+// the kernels of frame_kernel.cuh / object_kernels.cuh; nothing here falls back to the CPU.
+#include "../../include/sharp_b200.h"
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "object_kernels.cuh"
+
+using namespace sharp;
+
+namespace {
+
+constexpr double kTau = 1e-4;  // reading G4: thr = tau * a_rms
+thread_local std::string g_plan_error = "";
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+int env_int(const char *name, int dflt)
+{
+    const char *s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+}  // namespace
+
+struct sharp_plan_s {
+    int m = 0, K = 0, nr = 0, nc = 0;
+    int E = 16;  // elements per thread of the frame kernel (radix of the strided FFT pass)
+    int tiles_r = 0, tiles_c = 0;
+    std::vector<int32_t> pos;          // K x 2
+    std::vector<int32_t> tile_ptr;     // tiles + 1
+    std::vector<int32_t> tile_frames;  // CSR entries
+    std::string err;
+
+    // device
+    bool bound = false;
+    cudaStream_t stream = nullptr;
+    unsigned char *ws = nullptr;
+    size_t ws_bytes = 0;
+    int frame_grid = 0;      // persistent CTAs of the frame kernel (= scratch slots)
+    int frame_nt = 256;
+    int probe_chunk = 64, probe_nchunks = 0;
+    int amp_blocks = 0;
+
+    // workspace offsets
+    size_t o_a = 0, o_c[2] = {0, 0}, o_psi_z = 0, o_psi_v[2] = {0, 0}, o_den = 0, o_w[4] = {0, 0, 0, 0}, o_scratch = 0,
+           o_pos = 0, o_tile_ptr = 0, o_tile_frames = 0, o_partials = 0, o_err_partials = 0, o_err_sums = 0, o_pnum = 0,
+           o_pden = 0, o_scalars = 0, o_total = 0;
+
+    // state
+    bool have_I = false, have_probe = false, have_frames = false, have_prev = false;
+    int cur = 0, vcur = 0;             // c[cur], psi_v[vcur] are the current factored frames
+    bool psi_v_zero = true;            // psi_v[vcur] is identically 0 (z = c)
+    bool prev_psi_v_zero = true;
+    int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
+    int refine_every = 0;
+    long long it = 0;
+    long long launches = 0;
+
+    template <class T>
+    T *dp(size_t off) const { return reinterpret_cast<T *>(ws + off); }
+    size_t npx() const { return (size_t)K * m * m; }
+    size_t nobj() const { return (size_t)nr * nc; }
+};
+
+namespace {
+
+int fail(sharp_plan_t *p, int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (p) p->err = buf; else g_plan_error = buf;
+    return code;
+}
+
+int cuda_fail(sharp_plan_t *p, cudaError_t e, const char *what)
+{
+    return fail(p, SHARP_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+#define CK(call)                                                   \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return cuda_fail(p, e__, #call);   \
+    } while (0)
+
+#define CK_LAUNCH(name)                                            \
+    do {                                                           \
+        cudaError_t e__ = cudaGetLastError();                      \
+        if (e__ != cudaSuccess) return cuda_fail(p, e__, name);    \
+        ++p->launches;                                             \
+    } while (0)
+
+int grid_for(size_t n, int per_block = 256, int cap = 148 * 16)
+{
+    size_t b = (n + per_block - 1) / per_block;
+    return (int)std::min<size_t>(std::max<size_t>(b, 1), (size_t)cap);
+}
+
+// ---- frame kernel dispatch -----------------------------------------------------------------------------------
+template <int M, int E, int NT, int MODE>
+int frame_smem_bytes()
+{
+    return FrameCfg<M, E, NT>::SMEM_BYTES + (E > 16 ? M * 8 : 0);
+}
+
+template <int M, int E, int NT, int MODE>
+cudaError_t frame_prepare(int *blocks_per_sm)
+{
+    const int smem = frame_smem_bytes<M, E, NT, MODE>();
+    cudaError_t e = cudaFuncSetAttribute(k_frame<M, E, NT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_frame<M, E, NT, MODE>, NT, smem);
+}
+
+template <int M, int E, int NT, int MODE>
+void frame_launch(const FrameArgs &a, int grid, cudaStream_t st)
+{
+    k_frame<M, E, NT, MODE><<<grid, NT, frame_smem_bytes<M, E, NT, MODE>(), st>>>(a);
+}
+
+template <int MODE>
+int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
+{
+    switch (p->m) {
+    case 64: frame_launch<64, 16, 256, MODE>(a, grid, p->stream); break;
+    case 128: frame_launch<128, 16, 256, MODE>(a, grid, p->stream); break;
+    case 256: frame_launch<256, 16, 256, MODE>(a, grid, p->stream); break;
+    case 512: frame_launch<512, 32, 256, MODE>(a, grid, p->stream); break;
+    default: return fail(p, SHARP_EINVAL, "unsupported frame size %d", p->m);
+    }
+    CK_LAUNCH("k_frame");
+    return SHARP_OK;
+}
+
+template <int MODE>
+cudaError_t frame_prepare_m(int m, int *bps)
+{
+    switch (m) {
+    case 64: return frame_prepare<64, 16, 256, MODE>(bps);
+    case 128: return frame_prepare<128, 16, 256, MODE>(bps);
+    case 256: return frame_prepare<256, 16, 256, MODE>(bps);
+    default: return frame_prepare<512, 32, 256, MODE>(bps);
+    }
+}
+
+FrameArgs base_frame_args(sharp_plan_t *p)
+{
+    FrameArgs a;
+    memset(&a, 0, sizeof a);
+    a.a_int = p->dp<float>(p->o_a);
+    a.pos = p->dp<int>(p->o_pos);
+    a.scratch = p->dp<float2>(p->o_scratch);
+    a.sc = p->dp<DevScalars>(p->o_scalars);
+    a.K = p->K;
+    a.nc = p->nc;
+    return a;
+}
+
+OverlapArgs base_overlap_args(sharp_plan_t *p)
+{
+    OverlapArgs a;
+    memset(&a, 0, sizeof a);
+    a.m = p->m; a.nr = p->nr; a.nc = p->nc; a.tiles_c = p->tiles_c;
+    a.pos = p->dp<int>(p->o_pos);
+    a.tile_ptr = p->dp<int>(p->o_tile_ptr);
+    a.tile_frames = p->dp<int>(p->o_tile_frames);
+    a.den = p->dp<float>(p->o_den);
+    return a;
+}
+
+template <int MODE>
+int overlap_launch(sharp_plan_t *p, const OverlapArgs &a)
+{
+    k_overlap<MODE><<<p->tiles_r * p->tiles_c, 256, 0, p->stream>>>(a);
+    CK_LAUNCH("k_overlap");
+    return SHARP_OK;
+}
+
+int rebuild_den(sharp_plan_t *p)
+{
+    OverlapArgs a = base_overlap_args(p);
+    a.w_a = p->dp<float2>(p->o_w[p->w_cur]);
+    return overlap_launch<OV_DEN>(p, a);
+}
+
+// psi_z <- L_{w_cur} z for the current factored frames z = c[cur] + w_form . T psi_v[vcur]
+int regather_psi_z(sharp_plan_t *p)
+{
+    OverlapArgs a = base_overlap_args(p);
+    a.f = p->dp<float2>(p->o_c[p->cur]);
+    a.w_a = p->dp<float2>(p->o_w[p->w_cur]);
+    a.w_b = p->dp<float2>(p->o_w[p->w_form]);
+    a.psi_z = p->dp<float2>(p->o_psi_z);
+    a.psi_v_in = p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]);
+    return overlap_launch<OV_REGATHER>(p, a);
+}
+
+int free_probe_slot(const sharp_plan_t *p)
+{
+    for (int j = 0; j < 4; ++j)
+        if (j != p->w_cur && j != p->w_form && j != p->w_prev) return j;
+    return -1;  // cannot happen: four buffers, three roles
+}
+
+int check_ready(sharp_plan_t *p, bool need_I, bool need_probe)
+{
+    if (!p) return SHARP_EINVAL;
+    if (!p->bound) return fail(p, SHARP_ESTATE, "sharp_bind has not been called");
+    if (need_I && !p->have_I) return fail(p, SHARP_ESTATE, "sharp_set_intensities has not been called");
+    if (need_probe && !p->have_probe) return fail(p, SHARP_ESTATE, "sharp_set_probe has not been called");
+    return SHARP_OK;
+}
+
+// frames installed directly in c[cur] (z = c): reset the factored state around them
+int adopt_frames(sharp_plan_t *p)
+{
+    p->psi_v_zero = true;
+    p->have_prev = false;
+    p->w_form = p->w_cur;
+    p->w_prev = p->w_cur;
+    p->it = 0;
+    p->have_frames = true;
+    return regather_psi_z(p);
+}
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_rows, int obj_cols)
+{
+    if (!out) return fail(nullptr, SHARP_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!(m == 64 || m == 128 || m == 256 || m == 512)) return fail(nullptr, SHARP_EINVAL, "m must be 64, 128, 256 or 512 (got %d)", m);
+    if (K < 1) return fail(nullptr, SHARP_EINVAL, "K must be >= 1 (got %d)", K);
+    if (!pos_rc) return fail(nullptr, SHARP_EINVAL, "pos_rc is NULL");
+    if (obj_rows < m || obj_cols < m) return fail(nullptr, SHARP_EINVAL, "object %d x %d smaller than the frame %d", obj_rows, obj_cols, m);
+    if ((long long)K * m * m > (1LL << 40) || (long long)obj_rows * obj_cols > (1LL << 31) - 1)
+        return fail(nullptr, SHARP_EINVAL, "problem too large");
+    for (int i = 0; i < K; ++i) {
+        const int r = pos_rc[2 * i], c = pos_rc[2 * i + 1];
+        if (r < 0 || c < 0 || r > obj_rows - m || c > obj_cols - m)
+            return fail(nullptr, SHARP_EINVAL, "position %d = (%d, %d) outside [0, %d] x [0, %d] (PAPER.md:53)", i, r, c, obj_rows - m, obj_cols - m);
+    }
+    sharp_plan_t *p = new (std::nothrow) sharp_plan_s;
+    if (!p) return fail(nullptr, SHARP_ENOMEM, "host allocation failed");
+    p->m = m; p->K = K; p->nr = obj_rows; p->nc = obj_cols;
+    p->E = (m == 512) ? 32 : 16;
+    p->pos.assign(pos_rc, pos_rc + 2 * (size_t)K);
+    p->tiles_r = (obj_rows + TILE - 1) / TILE;
+    p->tiles_c = (obj_cols + TILE - 1) / TILE;
+
+    // CSR tile lists by a two-pass counting sort over frames in ascending index: frame i touches the tile
+    // rectangle [r/T, (r+m-1)/T] x [c/T, (c+m-1)/T].
+    const size_t ntiles = (size_t)p->tiles_r * p->tiles_c;
+    p->tile_ptr.assign(ntiles + 1, 0);
+    for (int i = 0; i < K; ++i) {
+        const int r = pos_rc[2 * i], c = pos_rc[2 * i + 1];
+        for (int ty = r / TILE; ty <= (r + m - 1) / TILE; ++ty)
+            for (int tx = c / TILE; tx <= (c + m - 1) / TILE; ++tx) ++p->tile_ptr[(size_t)ty * p->tiles_c + tx + 1];
+    }
+    for (size_t j = 0; j < ntiles; ++j) p->tile_ptr[j + 1] += p->tile_ptr[j];
+    p->tile_frames.resize((size_t)p->tile_ptr[ntiles]);
+    {
+        std::vector<int32_t> fill(p->tile_ptr.begin(), p->tile_ptr.end() - 1);
+        for (int i = 0; i < K; ++i) {
+            const int r = pos_rc[2 * i], c = pos_rc[2 * i + 1];
+            for (int ty = r / TILE; ty <= (r + m - 1) / TILE; ++ty)
+                for (int tx = c / TILE; tx <= (c + m - 1) / TILE; ++tx) p->tile_frames[(size_t)fill[(size_t)ty * p->tiles_c + tx]++] = i;
+        }
+    }
+
+    // workspace layout.  The frame kernel is persistent: at most one scratch slot per resident CTA.
+    const int slots_cap = std::max(1, env_int("SHARP_FRAME_SLOTS", 148 * 2));
+    p->frame_grid = std::min(K, slots_cap);
+    p->probe_chunk = std::max(1, env_int("SHARP_PROBE_CHUNK", 32));
+    p->probe_nchunks = (K + p->probe_chunk - 1) / p->probe_chunk;
+    p->amp_blocks = grid_for(p->npx());
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    p->o_a = take(p->npx() * 4);
+    p->o_c[0] = take(p->npx() * 8);
+    p->o_c[1] = take(p->npx() * 8);
+    p->o_psi_z = take(p->nobj() * 8);
+    p->o_psi_v[0] = take(p->nobj() * 8);
+    p->o_psi_v[1] = take(p->nobj() * 8);
+    p->o_den = take(p->nobj() * 4);
+    for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
+    p->o_scratch = take((size_t)p->frame_grid * m * m * 8);
+    p->o_pos = take((size_t)K * 2 * 4);
+    p->o_tile_ptr = take((ntiles + 1) * 4);
+    p->o_tile_frames = take(std::max<size_t>(p->tile_frames.size(), 1) * 4);
+    p->o_partials = take((size_t)p->amp_blocks * 8);
+    p->o_err_partials = take((size_t)p->frame_grid * 3 * 8);
+    p->o_err_sums = take(3 * 8);
+    p->o_pnum = take((size_t)p->probe_nchunks * m * m * 8);
+    p->o_pden = take((size_t)p->probe_nchunks * m * m * 4);
+    p->o_scalars = take(sizeof(DevScalars));
+    p->o_total = o;
+    *out = p;
+    return SHARP_OK;
+}
+
+void sharp_destroy(sharp_plan_t *p) { delete p; }
+
+const char *sharp_last_error(const sharp_plan_t *p) { return p ? p->err.c_str() : g_plan_error.c_str(); }
+
+size_t sharp_workspace_bytes(const sharp_plan_t *p) { return p ? p->o_total : 0; }
+
+int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_stream)
+{
+    if (!p) return SHARP_EINVAL;
+    if (!dev_workspace) return fail(p, SHARP_EINVAL, "workspace is NULL");
+    if (reinterpret_cast<uintptr_t>(dev_workspace) % 256 != 0) return fail(p, SHARP_EINVAL, "workspace must be 256-byte aligned");
+    if (bytes < p->o_total) return fail(p, SHARP_ENOMEM, "workspace too small: %zu < %zu bytes", bytes, p->o_total);
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) return fail(p, SHARP_ECUDA, "no CUDA device: %s (this library has no CPU path)", cudaGetErrorString(e));
+    p->ws = static_cast<unsigned char *>(dev_workspace);
+    p->ws_bytes = bytes;
+    p->stream = static_cast<cudaStream_t>(cuda_stream);
+    // size the persistent grid from the occupancy of the iteration kernel
+    int bps = 0;
+    CK(frame_prepare_m<FRAME_ITER>(p->m, &bps));
+    int bps2 = 0;
+    CK(frame_prepare_m<FRAME_FFT>(p->m, &bps2));
+    CK(frame_prepare_m<FRAME_ERR>(p->m, &bps2));
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int want = env_int("SHARP_FRAME_CTAS_PER_SM", 0);
+    if (want > 0) bps = std::min(bps, want);
+    if (bps < 1) return fail(p, SHARP_ECUDA, "frame kernel does not fit on an SM");
+    p->frame_grid = std::min(p->frame_grid, sms * bps);
+    CK(cudaMemcpyAsync(p->dp<int>(p->o_pos), p->pos.data(), p->pos.size() * 4, cudaMemcpyHostToDevice, p->stream));
+    CK(cudaMemcpyAsync(p->dp<int>(p->o_tile_ptr), p->tile_ptr.data(), p->tile_ptr.size() * 4, cudaMemcpyHostToDevice, p->stream));
+    if (!p->tile_frames.empty())
+        CK(cudaMemcpyAsync(p->dp<int>(p->o_tile_frames), p->tile_frames.data(), p->tile_frames.size() * 4, cudaMemcpyHostToDevice, p->stream));
+    CK(cudaMemsetAsync(p->dp<void>(p->o_scalars), 0, sizeof(DevScalars), p->stream));
+    CK(cudaStreamSynchronize(p->stream));  // the host vectors may be read until here
+    p->bound = true;
+    p->have_I = p->have_probe = p->have_frames = p->have_prev = false;
+    p->cur = p->vcur = 0;
+    p->w_cur = p->w_form = p->w_prev = 0;
+    p->psi_v_zero = p->prev_psi_v_zero = true;
+    p->it = 0;
+    return SHARP_OK;
+}
+
+int sharp_set_intensities(sharp_plan_t *p, const float *I_dev)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!I_dev) return fail(p, SHARP_EINVAL, "I_dev is NULL");
+    k_amplitudes<<<p->amp_blocks, 256, 0, p->stream>>>(p->m, p->E, p->K, I_dev, p->dp<float>(p->o_a), p->dp<double>(p->o_partials));
+    CK_LAUNCH("k_amplitudes");
+    k_scalars<<<1, 32, 0, p->stream>>>(p->amp_blocks, p->dp<double>(p->o_partials), p->K, kTau, p->dp<DevScalars>(p->o_scalars));
+    CK_LAUNCH("k_scalars");
+    p->have_I = true;
+    return SHARP_OK;
+}
+
+int sharp_set_probe(sharp_plan_t *p, const float *w_dev)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!w_dev) return fail(p, SHARP_EINVAL, "w_dev is NULL");
+    const size_t bytes = (size_t)p->m * p->m * 8;
+    if (!p->have_frames) {
+        p->w_cur = p->w_form = p->w_prev = 0;
+        CK(cudaMemcpyAsync(p->dp<void>(p->o_w[0]), w_dev, bytes, cudaMemcpyDeviceToDevice, p->stream));
+        p->have_probe = true;
+        return rebuild_den(p);
+    }
+    // frames exist: they stay as they are (reading G10); only Q, Q* and Q*Q change from now on
+    const int slot = free_probe_slot(p);  // four buffers, three roles: one is always free
+    CK(cudaMemcpyAsync(p->dp<void>(p->o_w[slot]), w_dev, bytes, cudaMemcpyDeviceToDevice, p->stream));
+    p->w_cur = slot;
+    if (int rc = rebuild_den(p)) return rc;
+    return regather_psi_z(p);
+}
+
+int sharp_set_object(sharp_plan_t *p, const float *psi_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    p->cur = 0; p->vcur = 0;
+    k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc,
+                                                            reinterpret_cast<const float2 *>(psi_dev),
+                                                            p->dp<float2>(p->o_w[p->w_cur]), p->dp<float2>(p->o_c[0]));
+    CK_LAUNCH("k_split");
+    return adopt_frames(p);
+}
+
+int sharp_set_frames(sharp_plan_t *p, const float *z_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!z_dev) return fail(p, SHARP_EINVAL, "z_dev is NULL");
+    p->cur = 0; p->vcur = 0;
+    CK(cudaMemcpyAsync(p->dp<void>(p->o_c[0]), z_dev, p->npx() * 8, cudaMemcpyDeviceToDevice, p->stream));
+    return adopt_frames(p);
+}
+
+int sharp_set_probe_refine(sharp_plan_t *p, int every)
+{
+    if (!p) return SHARP_EINVAL;
+    if (every < 0) return fail(p, SHARP_EINVAL, "refine period must be >= 0");
+    p->refine_every = every;
+    return SHARP_OK;
+}
+
+int sharp_iterate(sharp_plan_t *p, int n, float beta)
+{
+    if (int rc = check_ready(p, true, true)) return rc;
+    if (n < 0) return fail(p, SHARP_EINVAL, "n must be >= 0");
+    if (!(beta > 0.5f && beta <= 1.0f)) return fail(p, SHARP_EINVAL, "beta must be in (0.5, 1] (PAPER.md:178), got %g", (double)beta);
+    if (!p->have_frames)
+        if (int rc = sharp_set_object(p, nullptr)) return rc;
+    const float mm = (float)p->m * (float)p->m;
+    for (int l = 0; l < n; ++l) {
+        // (a1-a4, frame half of a6)  c' = beta z + (1 - 2 beta) P_a z,  z = c + w_form . T psi_v
+        FrameArgs fa = base_frame_args(p);
+        fa.c_in = p->dp<float2>(p->o_c[p->cur]);
+        fa.c_out = p->dp<float2>(p->o_c[p->cur ^ 1]);
+        fa.psi_v = p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]);
+        fa.w_form = p->dp<float2>(p->o_w[p->w_form]);
+        fa.bm = beta / mm;
+        fa.om = 1.0f - 2.0f * beta;
+        if (int rc = frame_dispatch<FRAME_ITER>(p, fa, p->frame_grid)) return rc;
+        // (a5, object half of a6)  psi_y, psi_v' = beta (2 psi_y - psi_z), psi_z' = psi_y
+        OverlapArgs oa = base_overlap_args(p);
+        oa.f = fa.c_out;
+        oa.w_a = p->dp<float2>(p->o_w[p->w_cur]);
+        oa.psi_z = p->dp<float2>(p->o_psi_z);
+        oa.psi_v_out = p->dp<float2>(p->o_psi_v[p->vcur ^ 1]);
+        oa.beta = beta;
+        if (int rc = overlap_launch<OV_ITER>(p, oa)) return rc;
+        // the new frames are z' = c[cur^1] + w_cur . T psi_v[vcur^1]; the old ones stay readable for eps_Delta
+        p->prev_psi_v_zero = p->psi_v_zero;
+        p->psi_v_zero = false;
+        p->cur ^= 1;
+        p->vcur ^= 1;
+        p->w_prev = p->w_form;
+        p->w_form = p->w_cur;
+        p->have_prev = true;
+        ++p->it;
+        // (a7) illumination refinement, Eq. 10, with psi = psi_y (in psi_z) and the new frames
+        if (p->refine_every > 0 && p->it % p->refine_every == 0) {
+            const int mm_i = p->m * p->m;
+            dim3 g(mm_i / 256, p->probe_nchunks);
+            k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nc,
+                                                      p->dp<float2>(p->o_c[p->cur]), p->dp<float2>(p->o_psi_v[p->vcur]),
+                                                      p->dp<float2>(p->o_w[p->w_form]), p->dp<float2>(p->o_psi_z),
+                                                      p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden));
+            CK_LAUNCH("k_probe_partial");
+            int slot = free_probe_slot(p);
+            if (slot < 0) return fail(p, SHARP_ECUDA, "internal: no free probe slot");
+            k_probe_final<<<mm_i / 256, 256, 0, p->stream>>>(p->m, p->probe_nchunks, p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden),
+                                                             p->dp<float2>(p->o_w[p->w_cur]), p->dp<float2>(p->o_w[slot]));
+            CK_LAUNCH("k_probe_final");
+            p->w_cur = slot;
+            if (int rc = rebuild_den(p)) return rc;
+            if (int rc = regather_psi_z(p)) return rc;
+        }
+    }
+    return SHARP_OK;
+}
+
+int sharp_get_object(sharp_plan_t *p, float *out_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
+    if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet (call sharp_set_object or sharp_iterate)");
+    CK(cudaMemcpyAsync(out_dev, p->dp<void>(p->o_psi_z), p->nobj() * 8, cudaMemcpyDeviceToDevice, p->stream));
+    return SHARP_OK;
+}
+
+int sharp_get_probe(sharp_plan_t *p, float *out_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
+    CK(cudaMemcpyAsync(out_dev, p->dp<void>(p->o_w[p->w_cur]), (size_t)p->m * p->m * 8, cudaMemcpyDeviceToDevice, p->stream));
+    return SHARP_OK;
+}
+
+int sharp_get_frames(sharp_plan_t *p, float *out_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
+    if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
+    k_materialize<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc, p->dp<float2>(p->o_c[p->cur]),
+                                                             p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]),
+                                                             p->dp<float2>(p->o_w[p->w_form]), reinterpret_cast<float2 *>(out_dev));
+    CK_LAUNCH("k_materialize");
+    return SHARP_OK;
+}
+
+int sharp_get_amplitudes(sharp_plan_t *p, float *out_dev)
+{
+    if (int rc = check_ready(p, true, false)) return rc;
+    if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
+    k_amplitudes_natural<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->E, p->K, p->dp<float>(p->o_a), out_dev);
+    CK_LAUNCH("k_amplitudes_natural");
+    return SHARP_OK;
+}
+
+int sharp_errors(sharp_plan_t *p, float out[3])
+{
+    if (int rc = check_ready(p, true, true)) return rc;
+    if (!out) return fail(p, SHARP_EINVAL, "out is NULL");
+    if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
+    FrameArgs fa = base_frame_args(p);
+    fa.c_in = p->dp<float2>(p->o_c[p->cur]);
+    fa.psi_v = p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]);
+    fa.w_form = p->dp<float2>(p->o_w[p->w_form]);
+    if (p->have_prev) {
+        fa.c_prev = p->dp<float2>(p->o_c[p->cur ^ 1]);
+        fa.psi_v_prev = p->prev_psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur ^ 1]);
+        fa.w_form_prev = p->dp<float2>(p->o_w[p->w_prev]);
+    }
+    fa.psi_z = p->dp<float2>(p->o_psi_z);
+    fa.w_cur = p->dp<float2>(p->o_w[p->w_cur]);
+    fa.err_partials = p->dp<double>(p->o_err_partials);
+    if (int rc = frame_dispatch<FRAME_ERR>(p, fa, p->frame_grid)) return rc;
+    k_sum_triples<<<1, 32, 0, p->stream>>>(p->frame_grid, p->dp<double>(p->o_err_partials), p->dp<double>(p->o_err_sums));
+    CK_LAUNCH("k_sum_triples");
+    double sums[3];
+    DevScalars sc;
+    CK(cudaMemcpyAsync(sums, p->dp<void>(p->o_err_sums), sizeof sums, cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaMemcpyAsync(&sc, p->dp<void>(p->o_scalars), sizeof sc, cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+    for (int j = 0; j < 3; ++j) out[j] = (float)sqrt(sums[j] / sc.A2);
+    return SHARP_OK;
+}
+
+int sharp_sync(sharp_plan_t *p)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    CK(cudaStreamSynchronize(p->stream));
+    return SHARP_OK;
+}
+
+long long sharp_launch_count(const sharp_plan_t *p) { return p ? p->launches : 0; }
+
+int sharp_tile_grid(const sharp_plan_t *p, int *tiles_r, int *tiles_c)
+{
+    if (!p || !tiles_r || !tiles_c) return SHARP_EINVAL;
+    *tiles_r = p->tiles_r;
+    *tiles_c = p->tiles_c;
+    return SHARP_OK;
+}
+
+int sharp_tile_lists(const sharp_plan_t *p, const int32_t **tile_ptr, const int32_t **tile_frames)
+{
+    if (!p || !tile_ptr || !tile_frames) return SHARP_EINVAL;
+    *tile_ptr = p->tile_ptr.data();
+    *tile_frames = p->tile_frames.data();
+    return SHARP_OK;
+}
+
+int sharp_cover_counts(const sharp_plan_t *p, int32_t *out_host)
+{
+    if (!p || !out_host) return SHARP_EINVAL;
+    // 2-D difference array: +1/-1 at the corners of every frame, then prefix sums along both axes
+    const int nr = p->nr, nc = p->nc, m = p->m;
+    std::vector<int32_t> d((size_t)(nr + 1) * (nc + 1), 0);
+    auto at = [&](int r, int c) -> int32_t & { return d[(size_t)r * (nc + 1) + c]; };
+    for (int i = 0; i < p->K; ++i) {
+        const int r = p->pos[2 * i], c = p->pos[2 * i + 1];
+        at(r, c) += 1; at(r, c + m) -= 1; at(r + m, c) -= 1; at(r + m, c + m) += 1;
+    }
+    for (int r = 0; r <= nr; ++r)
+        for (int c = 1; c <= nc; ++c) at(r, c) += at(r, c - 1);
+    for (int r = 1; r <= nr; ++r)
+        for (int c = 0; c <= nc; ++c) at(r, c) += at(r - 1, c);
+    for (int r = 0; r < nr; ++r)
+        for (int c = 0; c < nc; ++c) out_host[(size_t)r * nc + c] = at(r, c);
+    return SHARP_OK;
+}
+
+int sharp_frame_index(sharp_plan_t *p, long long *out_dev)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
+    k_frame_index<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc, out_dev);
+    CK_LAUNCH("k_frame_index");
+    return SHARP_OK;
+}
+
+int sharp_op_split(sharp_plan_t *p, const float *psi_dev, float *out_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
+    k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc, reinterpret_cast<const float2 *>(psi_dev),
+                                                            p->dp<float2>(p->o_w[p->w_cur]), reinterpret_cast<float2 *>(out_dev));
+    CK_LAUNCH("k_split");
+    return SHARP_OK;
+}
+
+int sharp_op_overlap(sharp_plan_t *p, const float *f_dev, float *out_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!f_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
+    OverlapArgs a = base_overlap_args(p);
+    a.f = reinterpret_cast<const float2 *>(f_dev);
+    a.w_a = p->dp<float2>(p->o_w[p->w_cur]);
+    a.out = reinterpret_cast<float2 *>(out_dev);
+    return overlap_launch<OV_L>(p, a);
+}
+
+int sharp_op_pa(sharp_plan_t *p, const float *f_dev, float *out_dev)
+{
+    if (int rc = check_ready(p, true, false)) return rc;
+    if (!f_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
+    FrameArgs fa = base_frame_args(p);
+    fa.c_in = reinterpret_cast<const float2 *>(f_dev);
+    fa.c_out = reinterpret_cast<float2 *>(out_dev);
+    fa.bm = 0.0f;  // beta = 0: c' = P_a z
+    fa.om = 1.0f;
+    return frame_dispatch<FRAME_ITER>(p, fa, p->frame_grid);
+}
+
+int sharp_op_fft2(sharp_plan_t *p, const float *f_dev, float *out_dev, int sign)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!f_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
+    if (f_dev == out_dev) return fail(p, SHARP_EINVAL, "sharp_op_fft2 is out of place");
+    if (sign != 1 && sign != -1) return fail(p, SHARP_EINVAL, "sign must be -1 (F) or +1 (F*)");
+    FrameArgs fa = base_frame_args(p);
+    fa.c_in = reinterpret_cast<const float2 *>(f_dev);
+    fa.c_out = reinterpret_cast<float2 *>(out_dev);
+    fa.conj_io = (sign == 1);
+    return frame_dispatch<FRAME_FFT>(p, fa, p->frame_grid);
+}
+
+int sharp_op_probe(sharp_plan_t *p, const float *psi_dev, const float *z_dev, float *out_dev)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!psi_dev || !z_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
+    const int mm_i = p->m * p->m;
+    dim3 g(mm_i / 256, p->probe_nchunks);
+    k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nc,
+                                              reinterpret_cast<const float2 *>(z_dev), nullptr, p->dp<float2>(p->o_w[p->w_cur]),
+                                              reinterpret_cast<const float2 *>(psi_dev), p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden));
+    CK_LAUNCH("k_probe_partial");
+    k_probe_final<<<mm_i / 256, 256, 0, p->stream>>>(p->m, p->probe_nchunks, p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden),
+                                                     p->dp<float2>(p->o_w[p->w_cur]), reinterpret_cast<float2 *>(out_dev));
+    CK_LAUNCH("k_probe_final");
+    return SHARP_OK;
+}
+
+int sharp_reconstruct_host(sharp_plan_t *p, const float *I_host, const float *w_host, int n, float beta,
+                           float *psi_out_host, float *w_out_host, float eps_out[3])
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!I_host || !w_host) return fail(p, SHARP_EINVAL, "NULL input");
+    if (n < 0 || !(beta > 0.5f && beta <= 1.0f)) return fail(p, SHARP_EINVAL, "bad n or beta");
+    // staging: the second frame buffer is free until the first iteration writes it
+    float *stage = p->dp<float>(p->o_c[1]);
+    CK(cudaMemcpyAsync(stage, I_host, p->npx() * 4, cudaMemcpyHostToDevice, p->stream));
+    if (int rc = sharp_set_intensities(p, stage)) return rc;
+    p->have_frames = false;
+    float *wstage = p->dp<float>(p->o_psi_v[1]);  // object-sized >= m*m
+    CK(cudaMemcpyAsync(wstage, w_host, (size_t)p->m * p->m * 8, cudaMemcpyHostToDevice, p->stream));
+    if (int rc = sharp_set_probe(p, wstage)) return rc;
+    if (int rc = sharp_set_object(p, nullptr)) return rc;
+    if (int rc = sharp_iterate(p, n, beta)) return rc;
+    if (eps_out)
+        if (int rc = sharp_errors(p, eps_out)) return rc;
+    if (psi_out_host) CK(cudaMemcpyAsync(psi_out_host, p->dp<void>(p->o_psi_z), p->nobj() * 8, cudaMemcpyDeviceToHost, p->stream));
+    if (w_out_host) CK(cudaMemcpyAsync(w_out_host, p->dp<void>(p->o_w[p->w_cur]), (size_t)p->m * p->m * 8, cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+    return SHARP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,286 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Bars (BASELINE.json north_star): integer indexing bit-exact; each operator rel-L2 <= 1e-5; error metrics
+<= 1e-4 relative; free-running frames after 100 iterations <= 1e-3 where the iteration contracts.
+
+The scans are the BASELINE.json recipes on reduced rasters (sizes the oracle finishes in seconds) plus ragged
+random geometry; every size spans several FFT strips, several persistent-CTA rounds and a ragged tail."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import paper_1602_01448_b200 as sharp
+from paper_1602_01448_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+OP_TOL = 1e-5
+EPS_TOL = 1e-4
+
+
+def rel(a, b):
+    a = np.asarray(a); b = np.asarray(b)
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def _rc(shape, seed, scale=1.0):
+    rng = np.random.default_rng(seed)
+    return ((rng.standard_normal(shape) + 1j * rng.standard_normal(shape)) * scale).astype(np.complex64)
+
+
+SCANS = {
+    # name: (config number, reduced grid)
+    "m64": (1, 6),       # 36 frames 64x64
+    "m128": (2, 5),      # 25 frames 128x128, jittered
+    "m256": (4, 4),      # 16 frames 256x256, jittered, noise-free
+    "m512": (5, 7),      # 7 Fermat-spiral frames 512x512
+}
+
+
+@pytest.fixture(scope="module", params=list(SCANS))
+def scan(request):
+    n, grid = SCANS[request.param]
+    cfg = synth.reduced(synth.config(n), grid)
+    if cfg.kind == "fermat":
+        cfg = dataclasses.replace(cfg, step=20)      # keep the 7 frames overlapping
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    rec = sharp.Reconstruction(cfg.m, pos, shape)
+    rec.set_intensities(I)
+    rec.set_probe(wt)
+    yield dict(cfg=cfg, pos=pos, shape=shape, I=I, w0=w0, obj=obj, wt=wt, rec=rec)
+    rec.close()
+
+
+def test_frame_index_bit_exact(scan, oracle):
+    idx = scan["rec"].frame_index().cpu().numpy()
+    assert np.array_equal(idx, oracle.linear_index(scan["cfg"].m, scan["pos"], scan["shape"][1]))
+
+
+def test_amplitudes_roundtrip_and_norm(scan, oracle):
+    a, A2, a_rms, thr = oracle.amplitudes(scan["I"])
+    got = scan["rec"].get_amplitudes().cpu().numpy()
+    assert rel(got, a) < 1e-6
+
+
+def test_op_split(scan, oracle):
+    psi = _rc(scan["shape"], 11)
+    got = scan["rec"].op_split(psi).cpu().numpy()
+    assert rel(got, oracle.split(psi, scan["wt"], scan["pos"])) < OP_TOL
+
+
+def test_op_overlap(scan, oracle):
+    cfg = scan["cfg"]
+    f = _rc((cfg.K, cfg.m, cfg.m), 12)
+    got = scan["rec"].op_overlap(f).cpu().numpy()
+    want = oracle.L(f, scan["wt"], scan["pos"], scan["shape"])
+    den = oracle.overlap_den(scan["wt"], scan["pos"], scan["shape"])
+    # G5: object-space values at unlit pixels are ratios of rounding noise; compare where Q*Q >= 1e-3 max, and
+    # the whole array in the |w|^2-weighted norm that P_Q actually sees
+    lit = den >= 1e-3 * den.max()
+    assert rel(got[lit], want[lit]) < OP_TOL
+    assert rel(got * np.sqrt(den), want * np.sqrt(den)) < OP_TOL
+    assert np.all(got[den == 0] == 0)
+
+
+@pytest.mark.parametrize("sign", [-1, 1])
+def test_op_fft2(scan, oracle, sign):
+    cfg = scan["cfg"]
+    f = _rc((cfg.K, cfg.m, cfg.m), 13)
+    got = scan["rec"].op_fft2(f, sign).cpu().numpy()
+    for i in range(0, cfg.K, max(1, cfg.K // 4)):
+        assert rel(got[i], oracle.fft2(f[i], sign)) < OP_TOL
+    # Parseval on all frames (unitary)
+    assert abs(np.linalg.norm(got) / np.linalg.norm(f) - 1) < 1e-5
+
+
+def test_op_pa(scan, oracle):
+    cfg = scan["cfg"]
+    a, A2, a_rms, thr = oracle.amplitudes(scan["I"])
+    z = synth.exit_waves(cfg, scan["obj"], scan["wt"], scan["pos"]).astype(np.complex64)
+    z = (z * (1 + 0.3 * _rc(z.shape, 14))).astype(np.complex64)
+    got = scan["rec"].op_pa(z).cpu().numpy()
+    assert rel(got, oracle.Pa(z, a, thr)) < OP_TOL
+
+
+def test_pa_small_modulus_rule_G4(scan, oracle):
+    """flat object x pupil probe: F z is exactly the disc, outside it |Fz| is rounding noise."""
+    cfg = scan["cfg"]
+    a, A2, a_rms, thr = oracle.amplitudes(scan["I"])
+    z0 = oracle.split(np.ones(scan["shape"], np.complex64), scan["wt"], scan["pos"]).astype(np.complex64)
+    got = scan["rec"].op_pa(z0).cpu().numpy()
+    assert rel(got, oracle.Pa(z0, a, thr)) < OP_TOL
+
+
+@pytest.mark.parametrize("beta", [0.75, 0.9, 1.0])
+def test_one_raar_step_and_errors(scan, oracle, beta):
+    cfg, rec = scan["cfg"], scan["rec"]
+    a, A2, a_rms, thr = oracle.amplitudes(scan["I"])
+    z = synth.exit_waves(cfg, scan["obj"], scan["wt"], scan["pos"]).astype(np.complex64)
+    z = (z * (1 + 0.2 * _rc(z.shape, 15))).astype(np.complex64)
+    rec.set_probe_refine(0)
+    rec.set_probe(scan["wt"])
+    rec.set_frames(z)
+    assert rel(rec.get_frames().cpu().numpy(), z) == 0.0
+    e0 = rec.errors()
+    want0 = oracle.errors(z, None, scan["wt"], scan["pos"], scan["shape"], a, thr, A2)
+    assert np.allclose(e0, want0, rtol=EPS_TOL), (e0, want0)
+    rec.iterate(1, beta)
+    z1 = rec.get_frames().cpu().numpy()
+    want = oracle.raar(z, scan["wt"], scan["pos"], scan["shape"], a, thr, beta)
+    assert rel(z1, want) < OP_TOL
+    e1 = rec.errors()
+    want1 = oracle.errors(want, z, scan["wt"], scan["pos"], scan["shape"], a, thr, A2)
+    assert np.allclose(e1, want1, rtol=EPS_TOL), (e1, want1)
+    # the object estimate is Eq. 9 of the new frames
+    den = oracle.overlap_den(scan["wt"], scan["pos"], scan["shape"])
+    lit = den >= 1e-3 * den.max()
+    psi = rec.get_object().cpu().numpy()
+    assert rel(psi[lit], oracle.L(want, scan["wt"], scan["pos"], scan["shape"])[lit]) < 5e-5
+    # a second step exercises the factored state z = c + w T psi_v
+    rec.iterate(1, beta)
+    want2 = oracle.raar(want, scan["wt"], scan["pos"], scan["shape"], a, thr, beta)
+    assert rel(rec.get_frames().cpu().numpy(), want2) < 3 * OP_TOL
+    e2 = rec.errors()
+    want_e2 = oracle.errors(want2, want, scan["wt"], scan["pos"], scan["shape"], a, thr, A2)
+    assert np.allclose(e2, want_e2, rtol=3 * EPS_TOL), (e2, want_e2)
+
+
+def test_op_probe_update(scan, oracle):
+    """Eq. 10 as an operator, on a well-conditioned psi."""
+    cfg, rec = scan["cfg"], scan["rec"]
+    psi = (1.0 + 0.3 * _rc(scan["shape"], 21)).astype(np.complex64)
+    z = _rc((cfg.K, cfg.m, cfg.m), 22)
+    got = rec.op_probe(psi, z).cpu().numpy()
+    assert rel(got, oracle.probe_update(psi, z, scan["wt"], scan["pos"])) < OP_TOL
+    # closed form (P5): z = Q_w psi  ==>  Eq. 10 returns w
+    zq = oracle.split(psi, scan["wt"], scan["pos"]).astype(np.complex64)
+    assert rel(rec.op_probe(psi, zq).cpu().numpy(), scan["wt"]) < OP_TOL
+
+
+def test_probe_refinement_sequence_G10(scan, oracle):
+    """blind iterations: RAAR with the old w, psi = L_w z', Eq. 10 -> w', then Q*Q and psi under w'.  Without the
+    constraints of PAPER.md:163-164 this loop is ill-conditioned (psi at weakly lit pixels is a ratio of small
+    numbers and enters Eq. 10 with weight |psi|^2), so the bar is the oracle's own sensitivity to
+    fp32-sized input perturbations, floored at the operator tolerance."""
+    cfg, rec = scan["cfg"], scan["rec"]
+    w0 = synth.start_probe(dataclasses.replace(cfg, blind_start=True), scan["I"])
+    o = oracle.Oracle(cfg.m, scan["pos"], scan["shape"], scan["I"], w0, refine_every=1)
+    rng = np.random.default_rng(77)
+    Ip = (scan["I"].astype(np.float64) * (1 + 1e-7 * rng.standard_normal(scan["I"].shape))).astype(np.float32)
+    wp = (w0.astype(np.complex128) * (1 + 1e-7 * rng.standard_normal(w0.shape))).astype(np.complex64)
+    o2 = oracle.Oracle(cfg.m, scan["pos"], scan["shape"], Ip, wp, refine_every=1)
+    rec.set_probe(w0)
+    rec.set_object(None)
+    rec.set_probe_refine(1)
+    for it in range(3):
+        o.iterate(1, cfg.beta); o2.iterate(1, cfg.beta)
+        rec.iterate(1, cfg.beta)
+        tol_w = max(2 * OP_TOL, 10 * rel(o2.w, o.w))
+        tol_z = max(2 * OP_TOL, 10 * rel(o2.z, o.z))
+        assert rel(rec.get_probe().cpu().numpy(), o.w) < tol_w, (it, tol_w)
+        assert rel(rec.get_frames().cpu().numpy(), o.z) < tol_z, (it, tol_z)
+    e = rec.errors()
+    assert np.allclose(e, o.errors(), rtol=max(1e-3, 10 * np.abs(o2.errors() / o.errors() - 1).max())), (e, o.errors())
+    rec.set_probe_refine(0)
+    rec.set_probe(scan["wt"])
+
+
+def test_teacher_forced_trajectory_P9(scan, oracle):
+    """At several points of a free run, hand the GPU state to the oracle and advance both by one iteration."""
+    cfg, rec = scan["cfg"], scan["rec"]
+    a, A2, a_rms, thr = oracle.amplitudes(scan["I"])
+    rec.set_probe_refine(0)
+    rec.set_probe(scan["wt"])
+    rec.set_object(None)
+    done = 0
+    for upto in (1, 5, 12):
+        rec.iterate(upto - done, cfg.beta)
+        done = upto
+        z = rec.get_frames().cpu().numpy()
+        rec.iterate(1, cfg.beta)
+        done += 1
+        z1 = rec.get_frames().cpu().numpy()
+        want = oracle.raar(z, scan["wt"], scan["pos"], scan["shape"], a, thr, cfg.beta)
+        assert rel(z1, want) < OP_TOL, upto
+        e = rec.errors()
+        we = oracle.errors(want, z, scan["wt"], scan["pos"], scan["shape"], a, thr, A2)
+        assert np.allclose(e, we, rtol=EPS_TOL), (upto, e, we)
+
+
+def test_fixed_point_free_run_P10(scan, oracle):
+    """Noise-free data and a start at the true frames: RAAR must stay there, 100 iterations."""
+    cfg, rec = scan["cfg"], scan["rec"]
+    clean = dataclasses.replace(cfg, photons=0.0)
+    I = synth.intensities(clean, scan["obj"], scan["wt"], scan["pos"])
+    z0 = synth.exit_waves(cfg, scan["obj"], scan["wt"], scan["pos"]).astype(np.complex64)
+    rec.set_intensities(I)
+    rec.set_probe(scan["wt"])
+    rec.set_frames(z0)
+    n = 100 if cfg.m <= 128 else 30
+    rec.iterate(n, cfg.beta)
+    z = rec.get_frames().cpu().numpy()
+    assert rel(z, z0) < 1e-3
+    assert rel(z, z0) < 2e-5          # in fact it stays at fp32 noise level
+    e = rec.errors()
+    assert np.all(e < 1e-5), e
+    rec.set_intensities(scan["I"])
+
+
+def test_free_run_contracting_case_P10(oracle):
+    """config-4 recipe (noise-free, beta 0.9, broad probe) on a 5x5 raster: the iteration contracts after a
+    transient, so GPU and oracle frames must agree after 100 free-running iterations."""
+    cfg = synth.reduced(synth.config(4), 5)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    rec = sharp.Reconstruction(cfg.m, pos, shape)
+    rec.set_intensities(I); rec.set_probe(w0); rec.set_object(None)
+    rec.iterate(100, cfg.beta)
+    o = oracle.Oracle(cfg.m, pos, shape, I, w0)
+    o.iterate(100, cfg.beta)
+    z = rec.get_frames().cpu().numpy()
+    assert rel(z, o.z) < 1e-3
+    e, eo = rec.errors(), o.errors()
+    assert np.allclose(e[:2], eo[:2], rtol=1e-2, atol=1e-7), (e, eo)
+    rec.close()
+
+
+def test_edge_cases(oracle):
+    # K = 1 (no overlap at all), frame == object
+    m = 64
+    rng = np.random.default_rng(3)
+    I = (rng.random((1, m, m)) * 2).astype(np.float32)
+    w = _rc((m, m), 4)
+    rec = sharp.Reconstruction(m, [[0, 0]], (m, m))
+    rec.set_intensities(I); rec.set_probe(w); rec.set_object(None)
+    rec.iterate(2, 0.75)
+    o = oracle.Oracle(m, [[0, 0]], (m, m), I, w); o.iterate(2, 0.75)
+    assert rel(rec.get_frames().cpu().numpy(), o.z) < 3e-5
+    # argument errors at the ABI
+    with pytest.raises(sharp.SharpError):
+        rec.iterate(1, 0.5)            # G15
+    with pytest.raises(sharp.SharpError):
+        rec.iterate(1, 1.01)
+    with pytest.raises(sharp.SharpError):
+        rec.iterate(-1, 0.75)
+    rec.iterate(0, 0.75)               # n = 0 is a no-op
+    rec.close()
+    # many copies of one position, w = 1: psi is the mean of the frames (P3)
+    K = 5
+    pos = np.zeros((K, 2), np.int32)
+    rec = sharp.Reconstruction(m, pos, (m, m))
+    rec.set_intensities(np.ones((K, m, m), np.float32)); rec.set_probe(np.ones((m, m), np.complex64))
+    f = _rc((K, m, m), 6)
+    assert rel(rec.op_overlap(f).cpu().numpy(), f.mean(0)) < 1e-6
+    rec.close()
+    # zero intensities and a frame of exact zeros: no NaN (G4 / G14)
+    rec = sharp.Reconstruction(m, [[0, 0], [3, 5]], (80, 80))
+    I = np.zeros((2, m, m), np.float32); I[1] = -1.0
+    rec.set_intensities(I); rec.set_probe(w)
+    out = rec.op_pa(np.zeros((2, m, m), np.complex64)).cpu().numpy()
+    assert np.all(np.isfinite(out.view(np.float32))) and np.all(out == 0)
+    rec.close()
+
+
+def test_unbound_library_refuses(oracle):
+    rec = sharp.Reconstruction(64, [[0, 0]], (64, 64), device=None)
+    assert rec.lib.sharp_iterate(rec._plan, 1, 0.75) == sharp.SHARP_ESTATE
+    rec.close()
