@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- RAAR frame-iterations/s of the SHARP projection loop (arXiv 1602.01448) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5|1] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one synthetic scan: z0 = Q psi0
+(split), `iters` RAAR iterations (fused FFT / magnitude projection / IFFT / frame combine + gather overlap with
+the object-space combine [+ Eq. 10 probe refinement on the blind configs]) and the three error norms.  The
+metric is frame-iterations/s = ranks * K_frames * iters * steps / time.
+
+  value      inputs resident in HBM when the timed region starts; CUDA events on the library's stream
+  e2e        the same metric through sharp_reconstruct_host: HOST (pinned) intensities and probe in, HOST object,
+             probe and residuals out, copies inside the timed region
+  roofline   the fused per-frame kernel: algorithmic bytes (20 B per frame pixel) / its average
+             launch duration, measured with CUDA events around each of its launches in a second pass over the
+             same steps, against MEASURED_PEAKS.json's HBM copy bandwidth
+  cpu_baseline / --impl reference   the CPU oracle (oracle/, double precision, OpenMP over the host cores) as it
+             stands, on a bounded sub-raster sample of the same recipe
+
+N > 1 (torchrun): every rank reconstructs its own scan (same recipe, seed + rank), no data-path collective:
+weak scaling.  Timing is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "RAAR frame-iterations/s"
+UNIT = "frame-iterations/s"
+BYTES_PER_PX_FRAME_KERNEL = 20          # read c (8) + read a (4) + write c' (8): SURVEY.md 8(d) "M20"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[n-1]; 2 = medium raster (default)")
+    ap.add_argument("--iters", type=int, default=0, help="RAAR iterations per step (0 = the config's own count)")
+    ap.add_argument("--grid", type=int, default=0, help="reduce the raster to grid x grid (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload(args, rank=0):
+    from paper_1602_01448_b200 import synth
+    cfg = synth.config(args.config)
+    if args.grid:
+        cfg = synth.reduced(cfg, args.grid)
+    if rank:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    iters = args.iters or cfg.iters
+    return cfg, iters
+
+
+def workload_name(cfg, iters):
+    return (f"{cfg.name}: {cfg.K} frames {cfg.m}x{cfg.m} c64, object {cfg.shape[0]}x{cfg.shape[1]}, "
+            f"beta {cfg.beta}, {iters} RAAR iterations/step, probe "
+            + (f"refined every {cfg.refine_every}" if cfg.refine_every else "fixed"))
+
+
+# ---- the CPU oracle, timed as it stands (cpu_baseline and --impl reference) ---------------------------------------
+def oracle_sample(args):
+    """A sub-raster of the same recipe that the oracle advances in a few seconds per step."""
+    from paper_1602_01448_b200 import synth
+    cfg = synth.config(args.config)
+    g = {64: 10, 128: 12, 256: 6, 512: 9}[cfg.m]          # frames: 100 / 144 / 36 / 9
+    scfg = synth.reduced(cfg, min(g, cfg.grid))
+    its = 2 if cfg.m <= 128 else 1
+    return scfg, its
+
+
+def time_oracle(args, steps, warmup):
+    from paper_1602_01448_b200 import synth
+    from oracle import sharp_oracle as orc
+    orc.build()
+    scfg, its = oracle_sample(args)
+    pos, shape, I, w0, obj, wt = synth.make(scfg)
+    o = orc.Oracle(scfg.m, pos, shape, I, w0, refine_every=scfg.refine_every)
+    for _ in range(warmup):
+        o.iterate(its, scfg.beta)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.iterate(its, scfg.beta)
+    dt = time.perf_counter() - t0
+    eps = o.errors()
+    return dict(value=scfg.K * its * steps / dt, unit=UNIT, cores=orc.n_threads(), kind="oracle",
+                sample=f"{scfg.K} frames {scfg.m}x{scfg.m} ({scfg.name}, same recipe), {its} RAAR iteration(s)/step, "
+                       f"{steps} timed steps after {warmup} warm-up, C double precision + OpenMP",
+                seconds=dt, ms_per_step=1e3 * dt / steps, eps=[float(e) for e in eps]), scfg, its
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg, iters = workload(args)
+    base, scfg, its = time_oracle(args, args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": base["ms_per_step"], "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, iters), "timed_sample": base["sample"]},
+        "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---- clocks during the timed region -------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.FIELDS}",
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.f.read().splitlines():
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 8:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # "under load": samples drawing more than half of the peak power seen
+        pmax = max(power)
+        load = [s for s, pw in zip(sm, power) if pw >= 0.5 * pmax] or sm
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": max(smax), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": pmax}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# ---- our arm ----------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import paper_1602_01448_b200 as sharp
+    from paper_1602_01448_b200 import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU path (use --impl reference for the oracle)")
+    sharp.load_library()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg, iters = workload(args, rank)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    K, m = cfg.K, cfg.m
+    I_host = torch.from_numpy(np.ascontiguousarray(I)).pin_memory()
+    w_host = torch.from_numpy(np.ascontiguousarray(w0)).pin_memory()
+    rec = sharp.Reconstruction(m, pos, shape, device=dev)
+    rec.set_probe_refine(cfg.refine_every)
+    I_dev = I_host.to(dev)
+    rec.set_intensities(I_dev)
+    w_dev = w_host.to(dev)
+    rec.set_probe(w_dev)
+
+    def step():
+        if cfg.refine_every:                 # the blind loop replaces the probe: every step restarts from w0
+            rec.set_probe(w_dev)
+        rec.set_object(None)                 # a1: z0 = Q psi0, flat start
+        rec.iterate(iters, cfg.beta)         # a2-a6 (+ a7 on blind configs)
+        return rec.errors()                  # a8 (synchronises)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(max(args.warmup, 3)):
+        eps = step()
+
+    # ---- timed region: device-resident ------------------------------------------------------------------------
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    l0 = rec.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        eps = step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = rec.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * K * iters * args.steps / (ms * 1e-3)
+
+    # ---- second pass over the same steps with events around every launch: per-kernel durations -----------------
+    rec.profile(True)
+    nprof = max(1, min(args.steps, 8192 // max(1, 2 * iters + 8)))
+    for _ in range(nprof):
+        step()
+    prof = rec.profile_read()
+    rec.profile(False)
+    f_ms, f_n = prof["frame"]
+    peak, peak_src = measured_peak()
+    alg_bytes = BYTES_PER_PX_FRAME_KERNEL * K * m * m
+    achieved = alg_bytes / (f_ms / f_n * 1e-3) / 1e9 if f_n else None
+    tot_ms = sum(v[0] for v in prof.values())
+    roofline = {
+        "kernel": "k_frame<FRAME_ITER> (fused split-add / FFT2 / magnitude projection / IFFT2 / frame combine)",
+        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "frac": (achieved / peak) if achieved else None, "traffic": None,
+        "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+        "avg_launch_ms": f_ms / f_n if f_n else None, "launches_timed": f_n,
+        "share_of_kernel_time": {k: (v[0] / tot_ms if tot_ms else None) for k, v in prof.items()},
+        "avg_ms": {k: (v[0] / v[1] if v[1] else None) for k, v in prof.items()},
+    }
+    traffic_file = os.path.join(ROOT, "profiles", f"traffic_cfg{args.config}.json")
+    if os.path.exists(traffic_file):         # dram bytes per launch read off a committed ncu --set full capture
+        try:
+            with open(traffic_file) as f:
+                roofline["traffic"] = json.load(f).get("frame_kernel_dram_bytes_per_launch")
+        except Exception:
+            pass
+
+    # ---- end to end: host buffers in, host buffers out ---------------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        n_e2e = max(1, min(args.steps, 5))
+        rec.reconstruct_host(I_host, w_host, iters, cfg.beta)      # warm-up (allocates the pinned outputs)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            psi, w, eps_h = rec.reconstruct_host(I_host, w_host, iters, cfg.beta)   # synchronous
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+        e2e = {"value": world * K * iters * n_e2e / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(I_host.numel() * 4 + w_host.numel() * 8),
+               "d2h_bytes_per_step": int(shape[0] * shape[1] * 8 + m * m * 8 + 12),
+               "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
+               "api": "sharp_reconstruct_host (pinned host intensities + probe in; object, probe, residuals out)"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        base, _, _ = time_oracle(args, steps=3, warmup=1)
+        cpu = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, iters), "config_number": args.config,
+                   "l2": "inputs larger than L2 (frame state 2x%.0f MB + amplitudes %.0f MB per iteration vs 126 MB L2)"
+                         % (K * m * m * 8 / 1e6, K * m * m * 4 / 1e6),
+                   "parallelism": "independent scan per GPU, no collective" if world > 1 else "single GPU",
+                   "step": "set_object(flat) + iterate(iters, beta) + errors()"},
+        "ms_per_iteration": ms / args.steps / iters,
+        "eps": [float(x) for x in eps],
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": roofline,
+        "e2e": e2e,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -111,6 +111,20 @@ int sharp_sync(sharp_plan_t *p);
 /* Number of kernels this plan has launched so far (bench.py's gpu_launches). */
 long long sharp_launch_count(const sharp_plan_t *p);
 
+/* Per-kernel device timing for the roofline report (bench.py).  sharp_profile(p, 1) synchronises, discards
+ * earlier records and from then on brackets every kernel launch of sharp_iterate with CUDA events on the bound
+ * stream; sharp_profile(p, 0) stops.  sharp_profile_read synchronises and returns, per kernel class, the summed
+ * event time (milliseconds) and the number of launches recorded (at most 8192 launches are recorded).
+ * Classes: FRAME = the fused per-frame FFT-project-IFFT-combine kernel of sharp_iterate; OVERLAP = the gather
+ * overlap + object-space RAAR epilogue of sharp_iterate; PROBE = the Eq. 10 partial-sum kernel; OTHER = the rest. */
+#define SHARP_PROF_FRAME 0
+#define SHARP_PROF_OVERLAP 1
+#define SHARP_PROF_PROBE 2
+#define SHARP_PROF_OTHER 3
+#define SHARP_PROF_NCLASS 4
+int sharp_profile(sharp_plan_t *p, int on);
+int sharp_profile_read(sharp_plan_t *p, double ms[SHARP_PROF_NCLASS], long long launches[SHARP_PROF_NCLASS]);
+
 /* ---- integer artefacts (compared bit-exactly with the oracle) ------------------------------
  * sharp_tile_grid: tiles_r x tiles_c tiles of SHARP_TILE^2 pixels.  sharp_tile_lists: HOST pointers (owned by the
  * plan) to the CSR arrays: tile_ptr[tiles_r*tiles_c + 1], tile_frames[tile_ptr[last]].

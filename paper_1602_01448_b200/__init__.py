@@ -39,6 +39,8 @@ _SIGNATURES = {
     "sharp_errors": (_i, [_vp, C.POINTER(_f)]),
     "sharp_sync": (_i, [_vp]),
     "sharp_launch_count": (_ll, [_vp]),
+    "sharp_profile": (_i, [_vp, _i]),
+    "sharp_profile_read": (_i, [_vp, C.POINTER(C.c_double), C.POINTER(_ll)]),
     "sharp_tile_grid": (_i, [_vp, C.POINTER(_i), C.POINTER(_i)]),
     "sharp_tile_lists": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
     "sharp_cover_counts": (_i, [_vp, _vp]),
@@ -210,6 +212,15 @@ class Reconstruction:
 
     def launch_count(self):
         return int(self.lib.sharp_launch_count(self._plan))
+
+    def profile(self, on):
+        self._check(self.lib.sharp_profile(self._plan, int(bool(on))))
+
+    def profile_read(self):
+        """{class: (summed ms, launches)} for the kernel classes of include/sharp_b200.h (SHARP_PROF_*)."""
+        ms, n = (C.c_double * 4)(), (_ll * 4)()
+        self._check(self.lib.sharp_profile_read(self._plan, ms, n))
+        return {k: (ms[j], int(n[j])) for j, k in enumerate(("frame", "overlap", "probe", "other"))}
 
     # integer artefacts
     def tile_grid(self):

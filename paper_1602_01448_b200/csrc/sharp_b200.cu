@@ -65,6 +65,11 @@ struct sharp_plan_s {
     long long it = 0;
     long long launches = 0;
 
+    // optional per-kernel timing (sharp_profile): CUDA events around the launches of each kernel class
+    bool profiling = false;
+    struct ProfSpan { int cls; cudaEvent_t beg, end; };
+    std::vector<ProfSpan> prof;
+
     template <class T>
     T *dp(size_t off) const { return reinterpret_cast<T *>(ws + off); }
     size_t npx() const { return (size_t)K * m * m; }
@@ -102,6 +107,23 @@ int cuda_fail(sharp_plan_t *p, cudaError_t e, const char *what)
         ++p->launches;                                             \
     } while (0)
 
+constexpr int kProfMaxSpans = 8192;
+
+// Brackets one launch with events on the plan's stream while profiling is on (no-op otherwise).
+struct ProfScope {
+    sharp_plan_t *p;
+    cudaEvent_t end = nullptr;
+    ProfScope(sharp_plan_t *plan, int cls) : p(plan)
+    {
+        if (!p->profiling || (int)p->prof.size() >= kProfMaxSpans) return;
+        cudaEvent_t b = nullptr;
+        if (cudaEventCreate(&b) != cudaSuccess || cudaEventCreate(&end) != cudaSuccess) { end = nullptr; return; }
+        cudaEventRecord(b, p->stream);
+        p->prof.push_back({cls, b, end});
+    }
+    ~ProfScope() { if (end) cudaEventRecord(end, p->stream); }
+};
+
 int grid_for(size_t n, int per_block = 256, int cap = 148 * 16)
 {
     size_t b = (n + per_block - 1) / per_block;
@@ -133,6 +155,7 @@ void frame_launch(const FrameArgs &a, int grid, cudaStream_t st)
 template <int MODE>
 int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
 {
+    ProfScope prof(p, MODE == FRAME_ITER ? SHARP_PROF_FRAME : SHARP_PROF_OTHER);
     switch (p->m) {
     case 64: frame_launch<64, 16, 256, MODE>(a, grid, p->stream); break;
     case 128: frame_launch<128, 16, 256, MODE>(a, grid, p->stream); break;
@@ -183,6 +206,7 @@ OverlapArgs base_overlap_args(sharp_plan_t *p)
 template <int MODE>
 int overlap_launch(sharp_plan_t *p, const OverlapArgs &a)
 {
+    ProfScope prof(p, MODE == OV_ITER ? SHARP_PROF_OVERLAP : SHARP_PROF_OTHER);
     k_overlap<MODE><<<p->tiles_r * p->tiles_c, 256, 0, p->stream>>>(a);
     CK_LAUNCH("k_overlap");
     return SHARP_OK;
@@ -314,7 +338,12 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     return SHARP_OK;
 }
 
-void sharp_destroy(sharp_plan_t *p) { delete p; }
+void sharp_destroy(sharp_plan_t *p)
+{
+    if (!p) return;
+    for (auto &s : p->prof) { cudaEventDestroy(s.beg); cudaEventDestroy(s.end); }
+    delete p;
+}
 
 const char *sharp_last_error(const sharp_plan_t *p) { return p ? p->err.c_str() : g_plan_error.c_str(); }
 
@@ -458,10 +487,13 @@ int sharp_iterate(sharp_plan_t *p, int n, float beta)
         if (p->refine_every > 0 && p->it % p->refine_every == 0) {
             const int mm_i = p->m * p->m;
             dim3 g(mm_i / 256, p->probe_nchunks);
-            k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nc,
-                                                      p->dp<float2>(p->o_c[p->cur]), p->dp<float2>(p->o_psi_v[p->vcur]),
-                                                      p->dp<float2>(p->o_w[p->w_form]), p->dp<float2>(p->o_psi_z),
-                                                      p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden));
+            {
+                ProfScope prof(p, SHARP_PROF_PROBE);
+                k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nc,
+                                                          p->dp<float2>(p->o_c[p->cur]), p->dp<float2>(p->o_psi_v[p->vcur]),
+                                                          p->dp<float2>(p->o_w[p->w_form]), p->dp<float2>(p->o_psi_z),
+                                                          p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden));
+            }
             CK_LAUNCH("k_probe_partial");
             int slot = free_probe_slot(p);
             if (slot < 0) return fail(p, SHARP_ECUDA, "internal: no free probe slot");
@@ -551,6 +583,31 @@ int sharp_sync(sharp_plan_t *p)
 }
 
 long long sharp_launch_count(const sharp_plan_t *p) { return p ? p->launches : 0; }
+
+int sharp_profile(sharp_plan_t *p, int on)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    CK(cudaStreamSynchronize(p->stream));
+    for (auto &s : p->prof) { cudaEventDestroy(s.beg); cudaEventDestroy(s.end); }
+    p->prof.clear();
+    p->profiling = on != 0;
+    return SHARP_OK;
+}
+
+int sharp_profile_read(sharp_plan_t *p, double ms[SHARP_PROF_NCLASS], long long launches[SHARP_PROF_NCLASS])
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!ms || !launches) return fail(p, SHARP_EINVAL, "NULL argument");
+    CK(cudaStreamSynchronize(p->stream));
+    for (int j = 0; j < SHARP_PROF_NCLASS; ++j) { ms[j] = 0.0; launches[j] = 0; }
+    for (auto &s : p->prof) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, s.beg, s.end));
+        ms[s.cls] += (double)t;
+        ++launches[s.cls];
+    }
+    return SHARP_OK;
+}
 
 int sharp_tile_grid(const sharp_plan_t *p, int *tiles_r, int *tiles_c)
 {
