@@ -12,6 +12,7 @@
 #include <string>
 #include <vector>
 
+#include "frame_smem.cuh"
 #include "object_kernels.cuh"
 
 using namespace sharp;
@@ -131,25 +132,20 @@ int grid_for(size_t n, int per_block = 256, int cap = 148 * 16)
 }
 
 // ---- frame kernel dispatch -----------------------------------------------------------------------------------
+// m = 64, 128: the frame lives in shared memory (frame_smem.cuh).  m = 256, 512: strips in shared memory, the
+// row<->column transposition through a per-CTA scratch in L2 (frame_kernel.cuh).
 template <int M, int E, int NT, int MODE>
 int frame_smem_bytes()
 {
     return FrameCfg<M, E, NT>::SMEM_BYTES + (E > 16 ? M * 8 : 0);
 }
 
-template <int M, int E, int NT, int MODE>
-cudaError_t frame_prepare(int *blocks_per_sm)
+template <class KernelT>
+cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int *blocks_per_sm)
 {
-    const int smem = frame_smem_bytes<M, E, NT, MODE>();
-    cudaError_t e = cudaFuncSetAttribute(k_frame<M, E, NT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_frame<M, E, NT, MODE>, NT, smem);
-}
-
-template <int M, int E, int NT, int MODE>
-void frame_launch(const FrameArgs &a, int grid, cudaStream_t st)
-{
-    k_frame<M, E, NT, MODE><<<grid, NT, frame_smem_bytes<M, E, NT, MODE>(), st>>>(a);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, kern, nt, smem);
 }
 
 template <int MODE>
@@ -157,10 +153,10 @@ int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
 {
     ProfScope prof(p, MODE == FRAME_ITER ? SHARP_PROF_FRAME : SHARP_PROF_OTHER);
     switch (p->m) {
-    case 64: frame_launch<64, 16, 256, MODE>(a, grid, p->stream); break;
-    case 128: frame_launch<128, 16, 256, MODE>(a, grid, p->stream); break;
-    case 256: frame_launch<256, 16, 256, MODE>(a, grid, p->stream); break;
-    case 512: frame_launch<512, 32, 256, MODE>(a, grid, p->stream); break;
+    case 64: k_frame_smem<64, 256, MODE><<<grid, 256, SmemFrameCfg<64, 256>::SMEM_BYTES, p->stream>>>(a); break;
+    case 128: k_frame_smem<128, 512, MODE><<<grid, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, p->stream>>>(a); break;
+    case 256: k_frame<256, 16, 256, MODE><<<grid, 256, frame_smem_bytes<256, 16, 256, MODE>(), p->stream>>>(a); break;
+    case 512: k_frame<512, 32, 256, MODE><<<grid, 256, frame_smem_bytes<512, 32, 256, MODE>(), p->stream>>>(a); break;
     default: return fail(p, SHARP_EINVAL, "unsupported frame size %d", p->m);
     }
     CK_LAUNCH("k_frame");
@@ -171,10 +167,10 @@ template <int MODE>
 cudaError_t frame_prepare_m(int m, int *bps)
 {
     switch (m) {
-    case 64: return frame_prepare<64, 16, 256, MODE>(bps);
-    case 128: return frame_prepare<128, 16, 256, MODE>(bps);
-    case 256: return frame_prepare<256, 16, 256, MODE>(bps);
-    default: return frame_prepare<512, 32, 256, MODE>(bps);
+    case 64: return kernel_prepare(k_frame_smem<64, 256, MODE>, 256, SmemFrameCfg<64, 256>::SMEM_BYTES, bps);
+    case 128: return kernel_prepare(k_frame_smem<128, 512, MODE>, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, bps);
+    case 256: return kernel_prepare(k_frame<256, 16, 256, MODE>, 256, frame_smem_bytes<256, 16, 256, MODE>(), bps);
+    default: return kernel_prepare(k_frame<512, 32, 256, MODE>, 256, frame_smem_bytes<512, 32, 256, MODE>(), bps);
     }
 }
 
@@ -323,7 +319,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->o_psi_v[1] = take(p->nobj() * 8);
     p->o_den = take(p->nobj() * 4);
     for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
-    p->o_scratch = take((size_t)p->frame_grid * m * m * 8);
+    p->o_scratch = take(m <= 128 ? 256 : (size_t)p->frame_grid * m * m * 8);   // m <= 128 keeps the frame in shared memory
     p->o_pos = take((size_t)K * 2 * 4);
     p->o_tile_ptr = take((ntiles + 1) * 4);
     p->o_tile_frames = take(std::max<size_t>(p->tile_frames.size(), 1) * 4);
