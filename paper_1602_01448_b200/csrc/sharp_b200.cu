@@ -12,7 +12,7 @@
 #include <string>
 #include <vector>
 
-#include "frame_smem.cuh"
+#include "frame_ws.cuh"
 #include "object_kernels.cuh"
 
 using namespace sharp;
@@ -63,6 +63,7 @@ struct sharp_plan_s {
     bool prev_psi_v_zero = true;
     int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
     int refine_every = 0;
+    bool use_ws = true;                // m = 128: warp-specialised iteration kernel (SHARP_FRAME_WS=0 disables)
     long long it = 0;
     long long launches = 0;
 
@@ -154,7 +155,12 @@ int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
     ProfScope prof(p, MODE == FRAME_ITER ? SHARP_PROF_FRAME : SHARP_PROF_OTHER);
     switch (p->m) {
     case 64: k_frame_smem<64, 256, MODE><<<grid, 256, SmemFrameCfg<64, 256>::SMEM_BYTES, p->stream>>>(a); break;
-    case 128: k_frame_smem<128, 512, MODE><<<grid, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, p->stream>>>(a); break;
+    case 128:
+        if (MODE == FRAME_ITER && p->use_ws)
+            k_frame_ws128<<<grid, WsCfg::NT, WsCfg::SMEM_BYTES, p->stream>>>(a);
+        else
+            k_frame_smem<128, 512, MODE><<<grid, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, p->stream>>>(a);
+        break;
     case 256: k_frame<256, 16, 256, MODE><<<grid, 256, frame_smem_bytes<256, 16, 256, MODE>(), p->stream>>>(a); break;
     case 512: k_frame<512, 32, 256, MODE><<<grid, 256, frame_smem_bytes<512, 32, 256, MODE>(), p->stream>>>(a); break;
     default: return fail(p, SHARP_EINVAL, "unsupported frame size %d", p->m);
@@ -168,7 +174,13 @@ cudaError_t frame_prepare_m(int m, int *bps)
 {
     switch (m) {
     case 64: return kernel_prepare(k_frame_smem<64, 256, MODE>, 256, SmemFrameCfg<64, 256>::SMEM_BYTES, bps);
-    case 128: return kernel_prepare(k_frame_smem<128, 512, MODE>, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, bps);
+    case 128: {
+        if (MODE == FRAME_ITER) {
+            cudaError_t e = kernel_prepare(k_frame_ws128, WsCfg::NT, WsCfg::SMEM_BYTES, bps);
+            if (e != cudaSuccess) return e;
+        }
+        return kernel_prepare(k_frame_smem<128, 512, MODE>, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, bps);
+    }
     case 256: return kernel_prepare(k_frame<256, 16, 256, MODE>, 256, frame_smem_bytes<256, 16, 256, MODE>(), bps);
     default: return kernel_prepare(k_frame<512, 32, 256, MODE>, 256, frame_smem_bytes<512, 32, 256, MODE>(), bps);
     }
@@ -279,6 +291,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     if (!p) return fail(nullptr, SHARP_ENOMEM, "host allocation failed");
     p->m = m; p->K = K; p->nr = obj_rows; p->nc = obj_cols;
     p->E = (m == 512) ? 32 : 16;
+    p->use_ws = env_int("SHARP_FRAME_WS", 1) != 0;
     p->pos.assign(pos_rc, pos_rc + 2 * (size_t)K);
     p->tiles_r = (obj_rows + TILE - 1) / TILE;
     p->tiles_c = (obj_cols + TILE - 1) / TILE;
