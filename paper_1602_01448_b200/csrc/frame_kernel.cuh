@@ -116,7 +116,22 @@ __device__ __forceinline__ void dft_b(float2 *v)
     for (int q = 0; q < E / RB; ++q) dft<RB, SGN>(v + q * RB);
 }
 
-template <int M, int E, int NT, int MODE>
+// Cluster helpers: the CS CTAs of a thread-block cluster share one frame (and one L2 scratch slot); strips are
+// dealt round-robin by cluster rank and the three stage changes are cluster barriers (release/acquire, so the
+// L2-resident scratch written with st.cg by one CTA is visible to the ld.cg of the others).
+__device__ __forceinline__ unsigned cluster_rank()
+{
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_barrier()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// Launched with cluster dimension CS (CS = 1: plain launch).  gridDim.x is a multiple of CS.
+template <int M, int E, int NT, int MODE, int CS>
 __global__ void __launch_bounds__(NT, (E <= 16 ? 2 : 1)) k_frame(FrameArgs A)
 {
     using C = FrameCfg<M, E, NT>;
@@ -134,17 +149,20 @@ __global__ void __launch_bounds__(NT, (E <= 16 ? 2 : 1)) k_frame(FrameArgs A)
     Twiddles<M, E> tw;
     tw.init(tw_tab, s, tid, NT);
 
-    float2 *scr = A.scratch + (size_t)blockIdx.x * M * M;
+    const int crank = CS > 1 ? (int)cluster_rank() : 0;
+    const int cid = blockIdx.x / CS, nclusters = gridDim.x / CS;
+    float2 *scr = A.scratch + (size_t)cid * M * M;
+    static_assert(C::NSTRIP % CS == 0, "strips must divide evenly over the cluster");
     const float thr2 = A.sc->thr2;
     const float bm = A.bm, om = A.om;
     double e_a = 0.0, e_q = 0.0, e_d = 0.0;
 
-    for (int i = blockIdx.x; i < A.K; i += gridDim.x) {
+    for (int i = cid; i < A.K; i += nclusters) {
         const int xr = A.pos[2 * i], xc = A.pos[2 * i + 1];
         const size_t fbase = (size_t)i * M * M;
 
         // ---------------- stage 1: rows.  form z, pass A, exchange, pass B, store transposed -------------
-        for (int sp = 0; sp < C::NSTRIP; ++sp) {
+        for (int sp = crank; sp < C::NSTRIP; sp += CS) {
             const int r0 = sp * L;
             float2 v[E];
             {
@@ -211,8 +229,9 @@ __global__ void __launch_bounds__(NT, (E <= 16 ? 2 : 1)) k_frame(FrameArgs A)
             __syncthreads();
         }
 
+        if (CS > 1) cluster_barrier();
         // ---------------- stage 2: columns (rows of the transposed scratch).  A, B, project, B^-1, A^-1 ----
-        for (int sp = 0; sp < C::NSTRIP; ++sp) {
+        for (int sp = crank; sp < C::NSTRIP; sp += CS) {
             const int p0 = sp * L;
             float2 v[E];
             {
@@ -305,11 +324,11 @@ __global__ void __launch_bounds__(NT, (E <= 16 ? 2 : 1)) k_frame(FrameArgs A)
                 for (int j = 0; j < E; ++j) st_l2(dst + s + j * TPL, v[j]);
             }
         }
-        __syncthreads();
+        if (CS > 1) cluster_barrier(); else __syncthreads();
 
         // ---------------- stage 3: rows.  load transposed, B^-1, exchange, A^-1, store c --------------------
         if constexpr (MODE == FRAME_ITER) {
-            for (int sp = 0; sp < C::NSTRIP; ++sp) {
+            for (int sp = crank; sp < C::NSTRIP; sp += CS) {
                 const int r0 = sp * L;
                 float2 v[E];
                 {
@@ -336,6 +355,7 @@ __global__ void __launch_bounds__(NT, (E <= 16 ? 2 : 1)) k_frame(FrameArgs A)
                 }
                 __syncthreads();
             }
+            if (CS > 1) cluster_barrier();   // the next frame's stage 1 overwrites the scratch the others still read
         }
     }
 

@@ -46,7 +46,8 @@ struct sharp_plan_s {
     cudaStream_t stream = nullptr;
     unsigned char *ws = nullptr;
     size_t ws_bytes = 0;
-    int frame_grid = 0;      // persistent CTAs of the frame kernel (= scratch slots)
+    int frame_grid = 0;      // persistent CTAs of the frame kernel
+    int slots_cap = 0;       // upper bound on frame_grid the workspace was sized for
     int frame_nt = 256;
     int probe_chunk = 64, probe_nchunks = 0;
     int amp_blocks = 0;
@@ -149,6 +150,29 @@ cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int *blocks_per_sm)
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, kern, nt, smem);
 }
 
+// m >= 256: CS CTAs of a cluster share one frame, so that the scratch slots in flight (one per cluster) stay
+// inside L2: 74 x 512 KB at m = 256, 18 x 2 MB at m = 512.
+constexpr int kCluster256 = 4, kCluster512 = 8;
+
+template <class KernelT>
+cudaError_t launch_cluster(KernelT kern, int grid, int nt, int smem, int cs, cudaStream_t st, const FrameArgs &a)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(nt);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cs;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
 template <int MODE>
 int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
 {
@@ -161,8 +185,14 @@ int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
         else
             k_frame_smem<128, 512, MODE><<<grid, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, p->stream>>>(a);
         break;
-    case 256: k_frame<256, 16, 256, MODE><<<grid, 256, frame_smem_bytes<256, 16, 256, MODE>(), p->stream>>>(a); break;
-    case 512: k_frame<512, 32, 256, MODE><<<grid, 256, frame_smem_bytes<512, 32, 256, MODE>(), p->stream>>>(a); break;
+    case 256:
+        CK(launch_cluster(k_frame<256, 16, 256, MODE, kCluster256>, grid, 256, frame_smem_bytes<256, 16, 256, MODE>(),
+                          kCluster256, p->stream, a));
+        break;
+    case 512:
+        CK(launch_cluster(k_frame<512, 32, 256, MODE, kCluster512>, grid, 256, frame_smem_bytes<512, 32, 256, MODE>(),
+                          kCluster512, p->stream, a));
+        break;
     default: return fail(p, SHARP_EINVAL, "unsupported frame size %d", p->m);
     }
     CK_LAUNCH("k_frame");
@@ -181,8 +211,8 @@ cudaError_t frame_prepare_m(int m, int *bps)
         }
         return kernel_prepare(k_frame_smem<128, 512, MODE>, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, bps);
     }
-    case 256: return kernel_prepare(k_frame<256, 16, 256, MODE>, 256, frame_smem_bytes<256, 16, 256, MODE>(), bps);
-    default: return kernel_prepare(k_frame<512, 32, 256, MODE>, 256, frame_smem_bytes<512, 32, 256, MODE>(), bps);
+    case 256: return kernel_prepare(k_frame<256, 16, 256, MODE, kCluster256>, 256, frame_smem_bytes<256, 16, 256, MODE>(), bps);
+    default: return kernel_prepare(k_frame<512, 32, 256, MODE, kCluster512>, 256, frame_smem_bytes<512, 32, 256, MODE>(), bps);
     }
 }
 
@@ -318,6 +348,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
 
     // workspace layout.  The frame kernel is persistent: at most one scratch slot per resident CTA.
     const int slots_cap = std::max(1, env_int("SHARP_FRAME_SLOTS", 148 * 2));
+    p->slots_cap = slots_cap;
     p->frame_grid = std::min(K, slots_cap);
     p->probe_chunk = std::max(1, env_int("SHARP_PROBE_CHUNK", 32));
     p->probe_nchunks = (K + p->probe_chunk - 1) / p->probe_chunk;
@@ -332,12 +363,14 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->o_psi_v[1] = take(p->nobj() * 8);
     p->o_den = take(p->nobj() * 4);
     for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
-    p->o_scratch = take(m <= 128 ? 256 : (size_t)p->frame_grid * m * m * 8);   // m <= 128 keeps the frame in shared memory
+    // m <= 128 keeps the frame in shared memory; above, one L2 scratch slot per cluster of CTAs
+    const int cs_plan = m == 256 ? 4 : 8;
+    p->o_scratch = take(m <= 128 ? 256 : (size_t)((slots_cap + cs_plan - 1) / cs_plan) * m * m * 8);
     p->o_pos = take((size_t)K * 2 * 4);
     p->o_tile_ptr = take((ntiles + 1) * 4);
     p->o_tile_frames = take(std::max<size_t>(p->tile_frames.size(), 1) * 4);
     p->o_partials = take((size_t)p->amp_blocks * 8);
-    p->o_err_partials = take((size_t)p->frame_grid * 3 * 8);
+    p->o_err_partials = take((size_t)slots_cap * 3 * 8);
     p->o_err_sums = take(3 * 8);
     p->o_pnum = take((size_t)p->probe_nchunks * m * m * 8);
     p->o_pden = take((size_t)p->probe_nchunks * m * m * 4);
@@ -382,7 +415,13 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     const int want = env_int("SHARP_FRAME_CTAS_PER_SM", 0);
     if (want > 0) bps = std::min(bps, want);
     if (bps < 1) return fail(p, SHARP_ECUDA, "frame kernel does not fit on an SM");
-    p->frame_grid = std::min(p->frame_grid, sms * bps);
+    if (p->m >= 256) {   // whole clusters only; one scratch slot per cluster
+        const int cs = p->m == 256 ? kCluster256 : kCluster512;
+        const long long want_ctas = std::min<long long>({(long long)p->K * cs, (long long)sms * bps, (long long)p->slots_cap});
+        p->frame_grid = (int)std::max<long long>(cs, want_ctas / cs * cs);
+    } else {
+        p->frame_grid = std::min(p->frame_grid, sms * bps);
+    }
     CK(cudaMemcpyAsync(p->dp<int>(p->o_pos), p->pos.data(), p->pos.size() * 4, cudaMemcpyHostToDevice, p->stream));
     CK(cudaMemcpyAsync(p->dp<int>(p->o_tile_ptr), p->tile_ptr.data(), p->tile_ptr.size() * 4, cudaMemcpyHostToDevice, p->stream));
     if (!p->tile_frames.empty())
