@@ -188,29 +188,62 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
         dn[k] = 0.f;
     }
 
-    for (int e = beg; e < end; ++e) {
-        const int fi = __ldg(A.tile_frames + e);
-        const int xr = __ldg(A.pos + 2 * fi), xc = __ldg(A.pos + 2 * fi + 1);
-        const int cc = pc - xc;
-        if ((unsigned)cc >= (unsigned)m) continue;
-        const float2 *fb = (MODE == OV_DEN) ? nullptr : A.f + (size_t)fi * m * m;
+    // The tile's list (frame index and position) is staged in shared memory in chunks, so the loads of the frame
+    // data do not hang off a chain of dependent index loads; UNR frames are in flight per thread at a time and
+    // are accumulated in list order (ascending frame index: reading G17).
+    constexpr int CH = 128, UNR = 4;
+    __shared__ int s_fi[CH], s_xr[CH], s_xc[CH];
+    for (int base = beg; base < end; base += CH) {
+        const int n = min(CH, end - base);
+        __syncthreads();
+        for (int j = threadIdx.x; j < n; j += blockDim.x) {
+            const int fi = __ldg(A.tile_frames + base + j);
+            s_fi[j] = fi;
+            s_xr[j] = __ldg(A.pos + 2 * fi);
+            s_xc[j] = __ldg(A.pos + 2 * fi + 1);
+        }
+        __syncthreads();
+        for (int e0 = 0; e0 < n; e0 += UNR) {
+            float2 fv[UNR][4], wa[UNR][4], wb[UNR][4];
+            bool ok[UNR][4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const int rr = pr0 + 8 * k - xr;
-            if ((unsigned)rr < (unsigned)m) {
-                const int off = rr * m + cc;
-                const float2 wa = __ldg(A.w_a + off);
-                if constexpr (MODE == OV_DEN) {
-                    dn[k] += wa.x * wa.x + wa.y * wa.y;
-                } else {
-                    const float2 fv = __ldcs(fb + off);
-                    // conj(wa) * fv
-                    num[k].x += wa.x * fv.x + wa.y * fv.y;
-                    num[k].y += wa.x * fv.y - wa.y * fv.x;
-                    if constexpr (MODE == OV_REGATHER) {
-                        const float2 wb = __ldg(A.w_b + off);
-                        cr[k].x += wa.x * wb.x + wa.y * wb.y;
-                        cr[k].y += wa.x * wb.y - wa.y * wb.x;
+            for (int u = 0; u < UNR; ++u) {
+                const int e = min(e0 + u, n - 1);
+                const int cc = pc - s_xc[e];
+                const bool colok = (e0 + u < n) && ((unsigned)cc < (unsigned)m);
+                const float2 *fb = (MODE == OV_DEN) ? nullptr : A.f + (size_t)s_fi[e] * m * m;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int rr = pr0 + 8 * k - s_xr[e];
+                    ok[u][k] = colok && ((unsigned)rr < (unsigned)m);
+                    const int off = rr * m + cc;
+                    wa[u][k] = make_float2(0.f, 0.f);
+                    fv[u][k] = make_float2(0.f, 0.f);
+                    wb[u][k] = make_float2(0.f, 0.f);
+                    if (ok[u][k]) {
+                        wa[u][k] = __ldg(A.w_a + off);
+                        if constexpr (MODE != OV_DEN) fv[u][k] = __ldcs(fb + off);
+                        if constexpr (MODE == OV_REGATHER) wb[u][k] = __ldg(A.w_b + off);
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    if (!ok[u][k]) continue;
+                    const float2 w_ = wa[u][k];
+                    if constexpr (MODE == OV_DEN) {
+                        dn[k] += w_.x * w_.x + w_.y * w_.y;
+                    } else {
+                        const float2 f_ = fv[u][k];
+                        num[k].x += w_.x * f_.x + w_.y * f_.y;   // conj(w_a) f
+                        num[k].y += w_.x * f_.y - w_.y * f_.x;
+                        if constexpr (MODE == OV_REGATHER) {
+                            const float2 b_ = wb[u][k];
+                            cr[k].x += w_.x * b_.x + w_.y * b_.y;
+                            cr[k].y += w_.x * b_.y - w_.y * b_.x;
+                        }
                     }
                 }
             }
