@@ -186,6 +186,21 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def max_over_ranks(x, dist, device):
+    """MAX of a scalar over all ranks (identity when not distributed)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, K, iters, steps, ms):
+    """whole-job frame-iterations/s: every rank advanced K frames by iters*steps iterations in `ms` (max over ranks)."""
+    return world * K * iters * steps / (ms * 1e-3)
+
+
 # ---- our arm ----------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
@@ -247,11 +262,8 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = rec.launch_count() - l0
     clocks = sampler.stop() if sampler else None
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * K * iters * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, dev)
+    value = job_value(world, K, iters, args.steps, ms)
 
     # ---- second pass over the same steps with events around every launch: per-kernel durations -----------------
     rec.profile(True)
@@ -293,10 +305,7 @@ def run_ours(args):
             psi, w, eps_h = rec.reconstruct_host(I_host, w_host, iters, cfg.beta)   # synchronous
         torch.cuda.synchronize(dev)
         dt = time.perf_counter() - t0
-        t = torch.tensor([dt], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt = float(t.item())
+        dt = max_over_ranks(dt, dist, dev)
         e2e = {"value": world * K * iters * n_e2e / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(I_host.numel() * 4 + w_host.numel() * 8),
                "d2h_bytes_per_step": int(shape[0] * shape[1] * 8 + m * m * 8 + 12),
