@@ -53,6 +53,7 @@ struct FrameArgs {
     float bm;                // beta / m^2
     float om;                // 1 - 2 beta
     int conj_io;             // FRAME_FFT: conjugate input and output (gives F*)
+    int stagger_ns;          // k_frame_ws128: delay of consumer group 1 at every stage start (phase staggering)
     // FRAME_ERR only
     const float2 *c_prev, *psi_v_prev, *w_form_prev;   // previous iterate in factored form (c_prev NULL: z_prev = 0)
     const float2 *psi_z, *w_cur;                        // P_Q z = w_cur . T psi_z
@@ -160,6 +161,13 @@ __global__ void __launch_bounds__(NT, (E <= 16 ? 2 : 1)) k_frame(FrameArgs A)
     for (int i = cid; i < A.K; i += nclusters) {
         const int xr = A.pos[2 * i], xc = A.pos[2 * i + 1];
         const size_t fbase = (size_t)i * M * M;
+        // the cluster's next frame (state and amplitudes) is pulled into L2 while this one is transformed
+        if (tid == 0 && crank == 0 && i + nclusters < A.K) {
+            const size_t nb = (size_t)(i + nclusters) * M * M;
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(A.c_in + nb), "r"(M * M * 8) : "memory");
+            if (MODE != FRAME_FFT)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(A.a_int + nb), "r"(M * M * 4) : "memory");
+        }
 
         // ---------------- stage 1: rows.  form z, pass A, exchange, pass B, store transposed -------------
         for (int sp = crank; sp < C::NSTRIP; sp += CS) {

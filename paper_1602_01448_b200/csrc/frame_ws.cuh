@@ -196,6 +196,7 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
     for (int i = blockIdx.x; i < A.K; i += gridDim.x, ++fseq) {
         const size_t fbase = (size_t)i * M * M;
 
+        if (g == 1 && A.stagger_ns > 0) __nanosleep(A.stagger_ns);
         // ---------------- stage 1: rows of this group.  staged z -> pass A -> exchange -> pass B ---------------
 #pragma unroll 1
         for (int u = 0; u < 2; ++u) {
@@ -238,6 +239,7 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
             }
         }
         named_bar_sync(3, C::NCONS);
+        if (g == 1 && A.stagger_ns > 0) __nanosleep(A.stagger_ns);
 
         // ---------------- stage 2: columns of this group.  X, Y (project), X^-1 ----------------------------------
 #pragma unroll 1
@@ -293,6 +295,7 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
             }
         }
         named_bar_sync(3, C::NCONS);
+        if (g == 1 && A.stagger_ns > 0) __nanosleep(A.stagger_ns);
 
         // ---------------- stage 3: rows of this group.  pass B^-1, exchange, pass A^-1, store c' -----------------
 #pragma unroll 1

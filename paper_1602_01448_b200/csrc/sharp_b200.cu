@@ -14,6 +14,7 @@
 
 #include "frame_ws.cuh"
 #include "object_kernels.cuh"
+#include "overlap_tma.cuh"
 
 using namespace sharp;
 
@@ -64,6 +65,8 @@ struct sharp_plan_s {
     bool prev_psi_v_zero = true;
     int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
     int refine_every = 0;
+    int stagger_ns = 0;                // SHARP_WS_STAGGER_NS: see FrameArgs::stagger_ns
+    bool use_tma_overlap = false;      // SHARP_OVERLAP_TMA=1 selects the TMA-box overlap (slower in round 1: w is not L1-cached)
     bool use_ws = true;                // m = 128: warp-specialised iteration kernel (SHARP_FRAME_WS=0 disables)
     long long it = 0;
     long long launches = 0;
@@ -226,6 +229,7 @@ FrameArgs base_frame_args(sharp_plan_t *p)
     a.sc = p->dp<DevScalars>(p->o_scalars);
     a.K = p->K;
     a.nc = p->nc;
+    a.stagger_ns = p->stagger_ns;
     return a;
 }
 
@@ -241,10 +245,54 @@ OverlapArgs base_overlap_args(sharp_plan_t *p)
     return a;
 }
 
+// ---- tensor maps for the TMA overlap (driver entry point resolved at run time: no link dependency on libcuda) ----
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = [] {
+        void *ptr = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            ptr = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(ptr);
+    }();
+    return fn;
+}
+
+// rank-3 map over K frames of m x m c64 (8-byte elements), or rank-2 over one m x m array; box TILE x TILE (x 1),
+// out-of-range coordinates read as zero.
+bool make_box_map(CUtensorMap *map, const void *base, int m, long long K)
+{
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const cuuint32_t rank = K > 0 ? 3 : 2;
+    cuuint64_t dims[3] = {(cuuint64_t)m, (cuuint64_t)m, (cuuint64_t)(K > 0 ? K : 1)};
+    cuuint64_t strides[2] = {(cuuint64_t)m * 8, (cuuint64_t)m * m * 8};
+    cuuint32_t box[3] = {OVT_BOXW, TILE, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, rank, const_cast<void *>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int MODE>
 int overlap_launch(sharp_plan_t *p, const OverlapArgs &a)
 {
     ProfScope prof(p, MODE == OV_ITER ? SHARP_PROF_OVERLAP : SHARP_PROF_OTHER);
+    if constexpr (MODE == OV_ITER || MODE == OV_L) {
+        if (p->use_tma_overlap) {
+            CUtensorMap mf, mw;
+            if (!make_box_map(&mf, a.f, p->m, p->K) || !make_box_map(&mw, a.w_a, p->m, 0))
+                return fail(p, SHARP_ECUDA, "cuTensorMapEncodeTiled failed");
+            k_overlap_tma<MODE><<<p->tiles_r * p->tiles_c, 256, OVT_SMEM_BYTES, p->stream>>>(a, mf, mw);
+            CK_LAUNCH("k_overlap_tma");
+            return SHARP_OK;
+        }
+    }
     k_overlap<MODE><<<p->tiles_r * p->tiles_c, 256, 0, p->stream>>>(a);
     CK_LAUNCH("k_overlap");
     return SHARP_OK;
@@ -322,6 +370,8 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->m = m; p->K = K; p->nr = obj_rows; p->nc = obj_cols;
     p->E = (m == 512) ? 32 : 16;
     p->use_ws = env_int("SHARP_FRAME_WS", 1) != 0;
+    p->stagger_ns = env_int("SHARP_WS_STAGGER_NS", 0);
+    p->use_tma_overlap = env_int("SHARP_OVERLAP_TMA", 0) != 0;
     p->pos.assign(pos_rc, pos_rc + 2 * (size_t)K);
     p->tiles_r = (obj_rows + TILE - 1) / TILE;
     p->tiles_c = (obj_cols + TILE - 1) / TILE;
@@ -409,6 +459,9 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     int bps2 = 0;
     CK(frame_prepare_m<FRAME_FFT>(p->m, &bps2));
     CK(frame_prepare_m<FRAME_ERR>(p->m, &bps2));
+    CK(cudaFuncSetAttribute(k_overlap_tma<OV_ITER>, cudaFuncAttributeMaxDynamicSharedMemorySize, OVT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_overlap_tma<OV_L>, cudaFuncAttributeMaxDynamicSharedMemorySize, OVT_SMEM_BYTES));
+    if (p->use_tma_overlap && !encode_tiled_fn()) p->use_tma_overlap = false;
     int dev = 0, sms = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
