@@ -1,0 +1,88 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (persistent grids of one
+CTA or cluster per SM slot, many rounds, ragged last round).
+
+config 2 (2,500 frames 128x128): one teacher-forced RAAR iteration of the whole scan against the oracle, all frames.
+config 4 size (10,000 frames 256x256): the oracle cannot run the whole scan, so the frame-local operators are
+compared on sampled frames the oracle computes one by one (F, F*, P_a), plus Parseval over all frames; the overlap
+is compared on sampled object pixels by brute force over the frame list."""
+import numpy as np
+import pytest
+import torch
+
+import paper_1602_01448_b200 as sharp
+from paper_1602_01448_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    a = np.asarray(a); b = np.asarray(b)
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def test_config2_full_one_iteration(oracle):
+    cfg = synth.config(2)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    rec = sharp.Reconstruction(cfg.m, pos, shape)
+    rec.set_intensities(I); rec.set_probe(w0); rec.set_object(None)
+    rec.iterate(3, cfg.beta)                       # reach a generic state with the factored form in use
+    z = rec.get_frames().cpu().numpy()
+    rec.iterate(1, cfg.beta)
+    z1 = rec.get_frames().cpu().numpy()
+    a, A2, a_rms, thr = oracle.amplitudes(I)
+    want = oracle.raar(z, w0, pos, shape, a, thr, cfg.beta)
+    assert rel(z1, want) < 1e-5
+    per_frame = np.linalg.norm((z1 - want).reshape(cfg.K, -1), axis=1) / np.linalg.norm(want.reshape(cfg.K, -1), axis=1)
+    assert per_frame.max() < 5e-5, (int(per_frame.argmax()), float(per_frame.max()))
+    e = rec.errors()
+    we = oracle.errors(want, z, w0, pos, shape, a, thr, A2)
+    assert np.allclose(e, we, rtol=1e-4), (e, we)
+    rec.close()
+
+
+def test_config4_size_sampled_operators(oracle):
+    cfg = synth.config(4)
+    pos = synth.positions(cfg)
+    K, m = cfg.K, cfg.m
+    rec = sharp.Reconstruction(m, pos, cfg.shape)
+    g = torch.Generator(device="cuda").manual_seed(1602)
+    I = torch.rand((K, m, m), device="cuda", generator=g) * 2.0
+    rec.set_intensities(I)
+    w = synth.true_probe(cfg)
+    rec.set_probe(w)
+    z = torch.view_as_complex(torch.randn((K, m, m, 2), device="cuda", generator=g))
+    sample = [0, 1, 147, 148, 2500, 7777, K - 2, K - 1]
+    # F and F*: sampled frames against the oracle's own FFT, Parseval on all frames
+    Z = rec.op_fft2(z, -1)
+    assert abs(float(torch.linalg.vector_norm(Z) / torch.linalg.vector_norm(z)) - 1) < 1e-5
+    for i in sample:
+        assert rel(Z[i].cpu().numpy(), oracle.fft2(z[i].cpu().numpy(), -1)) < 1e-5, i
+    Zi = rec.op_fft2(Z, +1)
+    assert float(torch.linalg.vector_norm(Zi - z) / torch.linalg.vector_norm(z)) < 1e-5
+    del Z, Zi
+    # P_a on sampled frames (amplitudes and threshold from the full intensity array)
+    y = rec.op_pa(z)
+    A2 = float(I.double().sum()); thr = 1e-4 * np.sqrt(A2 / (K * m * m))
+    for i in sample:
+        ai = np.sqrt(I[i].cpu().numpy().astype(np.float64))
+        assert rel(y[i].cpu().numpy(), oracle.Pa(z[i].cpu().numpy()[None], ai[None], thr)[0]) < 1e-5, i
+    del y
+    # overlap on sampled object pixels: brute force over all frames that cover the pixel, ascending index
+    psi = rec.op_overlap(z)
+    rng = np.random.default_rng(4)
+    w64 = w.astype(np.complex128)
+    for _ in range(24):
+        pr, pc = int(rng.integers(0, cfg.shape[0])), int(rng.integers(0, cfg.shape[1]))
+        rr, cc = pr - pos[:, 0], pc - pos[:, 1]
+        hit = np.nonzero((rr >= 0) & (rr < m) & (cc >= 0) & (cc < m))[0]
+        if hit.size == 0:
+            assert complex(psi[pr, pc]) == 0
+            continue
+        fv = torch.stack([z[int(i), int(rr[i]), int(cc[i])] for i in hit]).cpu().numpy().astype(np.complex128)
+        wv = w64[rr[hit], cc[hit]]
+        den = np.sum(np.abs(wv) ** 2)
+        if den < 1e-3:
+            continue                                # G5: ratio of rounding noise
+        want = np.sum(np.conj(wv) * fv) / den
+        assert abs(complex(psi[pr, pc]) - want) <= 2e-5 * max(abs(want), np.sqrt(np.sum(np.abs(fv) ** 2) / den) * 1e-1), (pr, pc)
+    rec.close()
