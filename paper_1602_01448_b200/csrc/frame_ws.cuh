@@ -4,21 +4,27 @@
 // of a6: z = c + w . T psi_v, FFT2, magnitude projection folded with the RAAR frame combine, IFFT2).  What is new
 // is who touches global memory:
 //
-//   * one PRODUCER warpgroup (4 warps, 64 registers/thread) forms z = c + w_form . T psi_v for the rows of the
-//     NEXT frame with fully coalesced 128-bit loads and writes them into a ring of six 16-row slots in shared
-//     memory (96 KB), signalling one mbarrier per slot.  It runs up to 96 rows ahead of the consumers, i.e. it
-//     works while they are in the column stage and the inverse row stage of the current frame, so none of the
+//   * one PRODUCER warpgroup (4 warps) stages z = c + w_form . T psi_v for the rows of the NEXT frame: the state c
+//     goes straight from global into the staging slot with cp.async (16-byte copies, no registers, all four rows
+//     of a warp in flight), the probe and the object tile come through registers with coalesced 128/64-bit loads,
+//     and each thread then combines in place the locations it copied itself.  Six 16-row chunks go to a ring in
+//     shared memory (96 KB, one full/empty mbarrier pair per slot), the last two (rows 96..127) in place into the
+//     frame buffer once the consumers have retired those rows, so a whole frame is staged ahead and none of the
 //     state / probe / object load latency is on the FFT warps' critical path;
-//   * four CONSUMER warpgroups (16 warps, 104 registers/thread, `setmaxnreg`) run the eight radix passes on the
-//     frame buffer F (128 KB).  They are split in two groups of 256 threads that own the row strips
-//     [64 g, 64 g + 64) in the row stages and the column strips with the same numbers in the column stage; passes
-//     inside a stage synchronise with a per-group named barrier only, the three stage changes with a
-//     consumer-wide one.
+//   * four CONSUMER warpgroups (16 warps) run the eight radix passes on the frame buffer F (128 KB).  They are
+//     split in two groups of 256 threads that own the row strips [64 g, 64 g + 64) in the row stages and the
+//     column strips with the same numbers in the column stage; passes inside a stage synchronise with a per-group
+//     named barrier only, the three stage changes with a consumer-wide one.  Group 1 runs its strips in the
+//     order (1, 0) in the inverse row stage so that rows 96..127 retire early.
+//   All 640 threads run at the launch budget of 96 registers (an earlier variant moved registers from the
+//   producer to the consumers with setmaxnreg; the pool of 640 x 96 left the consumers only 104, which bought
+//   nothing).
 //
-// Ring protocol: the eight 16-row chunks q of a frame are produced in the order j(q) the two groups consume them
-// (q = 0,1,4,5,2,3,6,7); chunk number n = 8 * frame_seq + j lives in slot n % 6; full[slot] (128 producer arrivals)
-// completes its (n / 6)-th phase when the chunk is written; empty[slot] (4 consumer-warp arrivals) completes it
-// when the four warps that read the chunk hold it in registers.
+// Ring protocol: chunk q of 16 rows has sequence number j(q) in the order the two groups consume them
+// (q = 0,1,4,5,2,3,6,7).  j < 6: slot j of the ring; full[j] (128 producer arrivals) completes its phase
+// `frame_seq` when the chunk is written, empty[j] (4 consumer-warp arrivals) when the four warps that read it hold
+// it in registers.  j = 6, 7: fullF[j - 6] likewise; emptyF (8 warp arrivals) completes when group 1 has read rows
+// 96..127 of the previous frame for the last time.
 #pragma once
 #include "frame_smem.cuh"
 
@@ -29,11 +35,8 @@ struct WsCfg {
     static constexpr int NCONS = 512, NPROD = 128, NT = NCONS + NPROD, GSZ = 256, L = 32;  // L: lines per group pass
     static constexpr int SR = 16, NSLOT = 6, CHUNKS = M / SR;                                // ring geometry
     static constexpr int F_BYTES = M * M * 8, S_BYTES = NSLOT * SR * M * 8;
-    static constexpr int SMEM_BYTES = F_BYTES + S_BYTES + 2 * NSLOT * 8;
-    // setmaxnreg moves registers inside the CTA's own pool (640 threads x 96 at launch = 61440), so the two
-    // budgets must satisfy 512 * REGS_CONS + 128 * REGS_PROD <= 61440 or the increase blocks for ever.
-    static constexpr int REGS_LAUNCH = 96, REGS_CONS = 104, REGS_PROD = 64;
-    static_assert(NCONS * REGS_CONS + NPROD * REGS_PROD <= NT * REGS_LAUNCH, "setmaxnreg budgets exceed the CTA pool");
+    static constexpr int SMEM_BYTES = F_BYTES + S_BYTES + (2 * NSLOT + 3) * 8;
+    static constexpr int REGS_LAUNCH = 96;   // 640 threads x 96 registers = 61440 of the SM's 65536
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -51,10 +54,10 @@ __device__ __forceinline__ bool mbar_try_wait(void *bar, unsigned parity)
     unsigned ok;
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(0x989680u)   // suspend-time hint (ns)
         : "memory");
     return ok != 0;
 }
@@ -62,23 +65,18 @@ __device__ __forceinline__ void mbar_wait(void *bar, unsigned parity)
 {
     // a protocol error must surface as a launch failure (SHARP_ECUDA), never as a hung GPU
     for (unsigned spins = 0; !mbar_try_wait(bar, parity); ++spins)
-        if (spins > (1u << 26)) __trap();
+        if (spins > (1u << 22)) __trap();
 }
+__device__ __forceinline__ void cp_async_16(void *smem_dst, const void *gmem_src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
-template <int N>
-__device__ __forceinline__ void reg_dec()
-{
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N));
-}
-template <int N>
-__device__ __forceinline__ void reg_inc()
-{
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
-}
-
 // production order of the eight 16-row chunks of a frame: position j -> chunk q, and its inverse
 __device__ __forceinline__ int ws_chunk_of(int j) { return (j & 1) | ((j & 2) << 1) | ((j & 4) >> 1); }
 __device__ __forceinline__ int ws_seq_of(int q) { return (q & 1) | ((q & 4) >> 1) | ((q & 2) << 1); }
@@ -92,6 +90,8 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
     float2 *S = reinterpret_cast<float2 *>(smem_raw + C::F_BYTES);
     unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + C::F_BYTES + C::S_BYTES);
     unsigned long long *empty = full + NSLOT;
+    unsigned long long *fullF = empty + NSLOT;   // [2]: chunks 6, 7 are produced in place in F rows 96..127
+    unsigned long long *emptyF = fullF + 2;      // group 1 has retired F rows 96..127 (8 warp arrivals)
 
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -99,20 +99,22 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
             mbar_init(full + k, C::NPROD);
             mbar_init(empty + k, 4);
         }
+        mbar_init(fullF + 0, C::NPROD);
+        mbar_init(fullF + 1, C::NPROD);
+        mbar_init(emptyF, 8);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
     if (tid >= C::NCONS) {
         // =========================== producer warpgroup ==================================================
-        reg_dec<C::REGS_PROD>();
         const int pw = (tid - C::NCONS) >> 5, lane = tid & 31;
         if (pw == 0 && lane == 0 && (int)blockIdx.x < A.K) {
             prefetch_l2_bulk(A.c_in + (size_t)blockIdx.x * M * M, M * M * 8);
             prefetch_l2_bulk(A.a_int + (size_t)blockIdx.x * M * M, M * M * 4);
         }
-        int n = 0;  // chunk counter of this CTA
-        for (int i = blockIdx.x; i < A.K; i += gridDim.x) {
+        int fseq = 0;  // frames this CTA has staged
+        for (int i = blockIdx.x; i < A.K; i += gridDim.x, ++fseq) {
             const int xr = A.pos[2 * i], xc = A.pos[2 * i + 1];
             const size_t fbase = (size_t)i * M * M;
             if (pw == 0 && lane == 0 && i + (int)gridDim.x < A.K) {
@@ -121,64 +123,69 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
                 prefetch_l2_bulk(A.a_int + nb, M * M * 4);
             }
 #pragma unroll 1
-            for (int j = 0; j < C::CHUNKS; ++j, ++n) {
-                const int slot = n % NSLOT, fill = n / NSLOT;
-                if (fill > 0) mbar_wait(empty + slot, (unsigned)((fill - 1) & 1));
+            for (int j = 0; j < C::CHUNKS; ++j) {
+                // chunks j = 0..5 go to ring slot j; j = 6, 7 (rows 96..127) in place into F once group 1 has
+                // retired those rows of the previous frame (it runs that strip first in stage 3)
+                const bool inF = j >= NSLOT;
+                if (fseq > 0) mbar_wait(inF ? emptyF : empty + j, (unsigned)((fseq - 1) & 1));
                 const int q = ws_chunk_of(j);
-                float2 *Sslot = S + slot * (SR * M);
+                float2 *Sslot = inF ? F + q * (SR * M) : S + j * (SR * M);
+                // this warp's rows 4 pw + {0..3} of the chunk; lane: pixels 2 lane, 2 lane + 1 and the same + 64.
+                // The state c goes straight into the slot with cp.async (no registers: all four rows in flight),
+                // the probe and the object tile through registers; each thread then combines in place the
+                // locations it copied itself, so no barrier is needed before the arrive.
 #pragma unroll
-                for (int half = 0; half < 2; ++half) {
-                    // this warp's rows 4 pw + 2 half + {0, 1} of the chunk; lane: pixels 2 lane, 2 lane + 1 and +64
-                    float4 cv[2][2], wv[2][2];
-                    float2 pv[2][4];
+                for (int rr = 0; rr < 4; ++rr) {
+                    const int rl = 4 * pw + rr, r = q * SR + rl;
+                    const float2 *crow = A.c_in + fbase + (size_t)r * M;
+                    float2 *drow = Sslot + rl * M;
+                    const int sw = swz_row(r);
+                    cp_async_16(drow + ((2 * lane) ^ sw), crow + 2 * lane);
+                    cp_async_16(drow + ((64 + 2 * lane) ^ sw), crow + 64 + 2 * lane);
+                }
+                cp_async_commit();
+                if (A.psi_v != nullptr) {
+                    float4 wv[4][2];
+                    float2 pv[4][4];
 #pragma unroll
-                    for (int rr = 0; rr < 2; ++rr) {
-                        const int rl = 4 * pw + 2 * half + rr, r = q * SR + rl;
-                        const float4 *c4 = reinterpret_cast<const float4 *>(A.c_in + fbase + (size_t)r * M);
-                        cv[rr][0] = __ldcs(c4 + lane);
-                        cv[rr][1] = __ldcs(c4 + 32 + lane);
+                    for (int rr = 0; rr < 4; ++rr) {
+                        const int r = q * SR + 4 * pw + rr;
+                        const float4 *w4 = reinterpret_cast<const float4 *>(A.w_form + r * M);
+                        wv[rr][0] = __ldg(w4 + lane);
+                        wv[rr][1] = __ldg(w4 + 32 + lane);
+                        const float2 *prow = A.psi_v + (size_t)(xr + r) * A.nc + xc;
+                        pv[rr][0] = __ldg(prow + 2 * lane);
+                        pv[rr][1] = __ldg(prow + 2 * lane + 1);
+                        pv[rr][2] = __ldg(prow + 64 + 2 * lane);
+                        pv[rr][3] = __ldg(prow + 64 + 2 * lane + 1);
                     }
-                    if (A.psi_v != nullptr) {
+                    cp_async_wait_all();
 #pragma unroll
-                        for (int rr = 0; rr < 2; ++rr) {
-                            const int rl = 4 * pw + 2 * half + rr, r = q * SR + rl;
-                            const float4 *w4 = reinterpret_cast<const float4 *>(A.w_form + r * M);
-                            wv[rr][0] = __ldg(w4 + lane);
-                            wv[rr][1] = __ldg(w4 + 32 + lane);
-                            const float2 *prow = A.psi_v + (size_t)(xr + r) * A.nc + xc;
-                            pv[rr][0] = __ldg(prow + 2 * lane);
-                            pv[rr][1] = __ldg(prow + 2 * lane + 1);
-                            pv[rr][2] = __ldg(prow + 64 + 2 * lane);
-                            pv[rr][3] = __ldg(prow + 64 + 2 * lane + 1);
-                        }
-#pragma unroll
-                        for (int rr = 0; rr < 2; ++rr)
-#pragma unroll
-                            for (int h = 0; h < 2; ++h) {
-                                const float2 z0 = cadd(make_float2(cv[rr][h].x, cv[rr][h].y),
-                                                       cmul(make_float2(wv[rr][h].x, wv[rr][h].y), pv[rr][2 * h]));
-                                const float2 z1 = cadd(make_float2(cv[rr][h].z, cv[rr][h].w),
-                                                       cmul(make_float2(wv[rr][h].z, wv[rr][h].w), pv[rr][2 * h + 1]));
-                                cv[rr][h] = make_float4(z0.x, z0.y, z1.x, z1.y);
-                            }
-                    }
-#pragma unroll
-                    for (int rr = 0; rr < 2; ++rr) {
-                        const int rl = 4 * pw + 2 * half + rr, r = q * SR + rl;
+                    for (int rr = 0; rr < 4; ++rr) {
+                        const int rl = 4 * pw + rr, r = q * SR + rl;
                         float4 *d4 = reinterpret_cast<float4 *>(Sslot + rl * M);
                         const int sw = swz_row(r);
-                        d4[((2 * lane) ^ sw) >> 1] = cv[rr][0];
-                        d4[((64 + 2 * lane) ^ sw) >> 1] = cv[rr][1];
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            float4 *slot4 = d4 + (((64 * h + 2 * lane) ^ sw) >> 1);
+                            const float4 cv = *slot4;
+                            const float2 z0 = cadd(make_float2(cv.x, cv.y),
+                                                   cmul(make_float2(wv[rr][h].x, wv[rr][h].y), pv[rr][2 * h]));
+                            const float2 z1 = cadd(make_float2(cv.z, cv.w),
+                                                   cmul(make_float2(wv[rr][h].z, wv[rr][h].w), pv[rr][2 * h + 1]));
+                            *slot4 = make_float4(z0.x, z0.y, z1.x, z1.y);
+                        }
                     }
+                } else {
+                    cp_async_wait_all();
                 }
-                mbar_arrive(full + slot);
+                mbar_arrive(inF ? fullF + (j - NSLOT) : full + j);
             }
         }
         return;
     }
 
     // =============================== consumer warpgroups ===================================================
-    reg_inc<C::REGS_CONS>();
     const int g = tid / C::GSZ, gtid = tid % C::GSZ;       // group, thread in group
     const int lineA = gtid / TPL, s = gtid % TPL;           // A / X mappings (32 lines, 8 threads each)
     const int lineB = gtid % L, t = gtid / L;               // B / Y mappings (32 lines, t in 0..7)
@@ -196,7 +203,6 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
     for (int i = blockIdx.x; i < A.K; i += gridDim.x, ++fseq) {
         const size_t fbase = (size_t)i * M * M;
 
-        if (g == 1 && A.stagger_ns > 0) __nanosleep(A.stagger_ns);
         // ---------------- stage 1: rows of this group.  staged z -> pass A -> exchange -> pass B ---------------
 #pragma unroll 1
         for (int u = 0; u < 2; ++u) {
@@ -205,15 +211,22 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
             {
                 const int r = r0 + lineA;
                 const int q = 4 * g + 2 * u + (warp_in_group >> 2);   // lineA / 16
-                const int n = fseq * C::CHUNKS + ws_seq_of(q);
-                const int slot = n % NSLOT;
-                mbar_wait(full + slot, (unsigned)((n / NSLOT) & 1));
-                const float2 *src = S + slot * (SR * M) + (lineA & (SR - 1)) * M;
+                const int j = ws_seq_of(q);
                 const int sw = swz_row(r);
+                if (j < NSLOT) {
+                    mbar_wait(full + j, (unsigned)(fseq & 1));
+                    const float2 *src = S + j * (SR * M) + (lineA & (SR - 1)) * M;
 #pragma unroll
-                for (int j = 0; j < E; ++j) v[j] = src[(s + j * TPL) ^ sw];
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty + slot);
+                    for (int jj = 0; jj < E; ++jj) v[jj] = src[(s + jj * TPL) ^ sw];
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty + j);
+                } else {   // rows 96..127: staged in place; the eight threads of a row sit in this warp
+                    mbar_wait(fullF + (j - NSLOT), (unsigned)(fseq & 1));
+                    const float2 *src = F + r * M;
+#pragma unroll
+                    for (int jj = 0; jj < E; ++jj) v[jj] = src[(s + jj * TPL) ^ sw];
+                    __syncwarp();
+                }
                 dft<E, -1>(v);
 #pragma unroll
                 for (int k = 1; k < E; ++k) v[k] = cmul(v[k], tw.get(k));
@@ -239,7 +252,6 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
             }
         }
         named_bar_sync(3, C::NCONS);
-        if (g == 1 && A.stagger_ns > 0) __nanosleep(A.stagger_ns);
 
         // ---------------- stage 2: columns of this group.  X, Y (project), X^-1 ----------------------------------
 #pragma unroll 1
@@ -295,11 +307,11 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
             }
         }
         named_bar_sync(3, C::NCONS);
-        if (g == 1 && A.stagger_ns > 0) __nanosleep(A.stagger_ns);
 
         // ---------------- stage 3: rows of this group.  pass B^-1, exchange, pass A^-1, store c' -----------------
 #pragma unroll 1
-        for (int u = 0; u < 2; ++u) {
+        for (int uu = 0; uu < 2; ++uu) {
+            const int u = uu ^ g;                           // group 1 retires rows 96..127 first (producer refills them)
             const int r0 = 64 * g + 32 * u;
             float2 v[E];
             {
@@ -324,6 +336,10 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
                 const int sw = swz_row(r);
 #pragma unroll
                 for (int k = 0; k < E; ++k) v[k] = row[(s + k * TPL) ^ sw];
+                if (g == 1 && uu == 0) {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(emptyF);
+                }
 #pragma unroll
                 for (int k = 1; k < E; ++k) v[k] = cmulc(v[k], tw.get(k));
                 dft<E, +1>(v);
@@ -332,6 +348,8 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
                 for (int j = 0; j < E; ++j) st_stream(dst + s + j * TPL, v[j]);
             }
         }
+        // group 1 ends stage 3 on the strip it starts the next frame's stage 1 with: its readers must be done
+        if (g == 1) named_bar_sync(bar_g, C::GSZ);
     }
 }
 
