@@ -154,8 +154,9 @@ cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int *blocks_per_sm)
 }
 
 // m >= 256: CS CTAs of a cluster share one frame, so that the scratch slots in flight (one per cluster) stay
-// inside L2: 74 x 512 KB at m = 256, 18 x 2 MB at m = 512.
-constexpr int kCluster256 = 4, kCluster512 = 8;
+// inside L2: 148 x 512 KB at m = 256, 18 x 2 MB at m = 512.  Measured at m = 256 (1,600 frames): 1 CTA per frame (296
+// slots, 155 MB: spills) 1.40 ms, clusters of 2 1.16 ms, clusters of 4 1.70 ms (barrier cost and imbalance).
+constexpr int kCluster256 = 2, kCluster512 = 8;
 
 template <class KernelT>
 cudaError_t launch_cluster(KernelT kern, int grid, int nt, int smem, int cs, cudaStream_t st, const FrameArgs &a)
@@ -414,7 +415,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->o_den = take(p->nobj() * 4);
     for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
     // m <= 128 keeps the frame in shared memory; above, one L2 scratch slot per cluster of CTAs
-    const int cs_plan = m == 256 ? 4 : 8;
+    const int cs_plan = m == 256 ? kCluster256 : kCluster512;
     p->o_scratch = take(m <= 128 ? 256 : (size_t)((slots_cap + cs_plan - 1) / cs_plan) * m * m * 8);
     p->o_pos = take((size_t)K * 2 * 4);
     p->o_tile_ptr = take((ntiles + 1) * 4);
