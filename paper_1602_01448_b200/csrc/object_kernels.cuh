@@ -141,14 +141,14 @@ __global__ void k_sum_triples(int n, const double *partials, double *out)
 // (reading G17).  256 threads, each owning one column and four rows (ty, ty+8, ty+16, ty+24) of the tile.
 //
 //   num(p)   = sum_i conj(w_a(p - x_i)) f_i(p - x_i)
-//   cross(p) = sum_i conj(w_a(p - x_i)) w_b(p - x_i)            (OV_REGATHER only)
+//   cross(p) = sum_i conj(w_a(p - x_i)) w_b(p - x_i)            (OV_DEN with w_b given: kept for OV_REGATHER)
 //   den(p)   = sum_i |w_a(p - x_i)|^2                            (OV_DEN only; otherwise read from the den array)
 // Epilogues:
-//   OV_DEN       den[p] = sum |w_a|^2
+//   OV_DEN       den[p] = sum |w_a|^2;  cross[p] = sum conj(w_a) w_b when w_b is given (no frame data touched)
 //   OV_L         out[p] = num/den, 0 where den == 0 (reading G5)
 //   OV_ITER      psi_c = num/den; psi_y = (psi_c - beta psi_z)/(1 - 2 beta); psi_v[p] = beta (2 psi_y - psi_z);
 //                psi_z[p] = psi_y                                (object half of RAAR)
-//   OV_REGATHER  psi_z[p] = (num + psi_v[p] cross)/den           (L_{w_a}(c + w_b . T psi_v) after w changed)
+//   OV_REGATHER  psi_z[p] = (num + psi_v[p] cross[p])/den        (L_{w_a}(c + w_b . T psi_v) after w changed)
 // ---------------------------------------------------------------------------------------------------------
 enum OverlapMode : int { OV_DEN = 0, OV_L = 1, OV_ITER = 2, OV_REGATHER = 3 };
 
@@ -159,7 +159,8 @@ struct OverlapArgs {
     const int *tile_frames;
     const float2 *f;        // K m m
     const float2 *w_a;      // m m
-    const float2 *w_b;      // m m (REGATHER)
+    const float2 *w_b;      // m m (DEN: second probe of the cross term, may be NULL)
+    float2 *cross;          // object-sized (DEN out when w_b given, REGATHER in)
     float *den;             // object-sized
     float2 *out;            // OV_L
     float2 *psi_z;          // ITER in/out, REGATHER out
@@ -223,7 +224,7 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
                     if (ok[u][k]) {
                         wa[u][k] = __ldg(A.w_a + off);
                         if constexpr (MODE != OV_DEN) fv[u][k] = __ldcs(fb + off);
-                        if constexpr (MODE == OV_REGATHER) wb[u][k] = __ldg(A.w_b + off);
+                        if constexpr (MODE == OV_DEN) { if (A.w_b != nullptr) wb[u][k] = __ldg(A.w_b + off); }
                     }
                 }
             }
@@ -235,15 +236,13 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
                     const float2 w_ = wa[u][k];
                     if constexpr (MODE == OV_DEN) {
                         dn[k] += w_.x * w_.x + w_.y * w_.y;
+                        const float2 b_ = wb[u][k];
+                        cr[k].x += w_.x * b_.x + w_.y * b_.y;     // conj(w_a) w_b (zero when w_b is absent)
+                        cr[k].y += w_.x * b_.y - w_.y * b_.x;
                     } else {
                         const float2 f_ = fv[u][k];
                         num[k].x += w_.x * f_.x + w_.y * f_.y;   // conj(w_a) f
                         num[k].y += w_.x * f_.y - w_.y * f_.x;
-                        if constexpr (MODE == OV_REGATHER) {
-                            const float2 b_ = wb[u][k];
-                            cr[k].x += w_.x * b_.x + w_.y * b_.y;
-                            cr[k].y += w_.x * b_.y - w_.y * b_.x;
-                        }
                     }
                 }
             }
@@ -258,6 +257,7 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
         const size_t p = (size_t)pr * A.nc + pc;
         if constexpr (MODE == OV_DEN) {
             A.den[p] = dn[k];
+            if (A.w_b != nullptr) A.cross[p] = cr[k];
         } else {
             const float d = A.den[p];
             const bool lit = d > 0.f;
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
                 float2 o = make_float2(0.f, 0.f);
                 if (lit) {
                     float2 t = num[k];
-                    if (A.psi_v_in != nullptr) t = cadd(t, cmul(A.psi_v_in[p], cr[k]));
+                    if (A.psi_v_in != nullptr) t = cadd(t, cmul(A.psi_v_in[p], A.cross[p]));
                     o = make_float2(t.x / d, t.y / d);
                 }
                 A.psi_z[p] = o;

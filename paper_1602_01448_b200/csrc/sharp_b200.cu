@@ -54,7 +54,7 @@ struct sharp_plan_s {
     int amp_blocks = 0;
 
     // workspace offsets
-    size_t o_a = 0, o_c[2] = {0, 0}, o_psi_z = 0, o_psi_v[2] = {0, 0}, o_den = 0, o_w[4] = {0, 0, 0, 0}, o_scratch = 0,
+    size_t o_a = 0, o_c[2] = {0, 0}, o_psi_z = 0, o_psi_v[2] = {0, 0}, o_den = 0, o_cross = 0, o_w[4] = {0, 0, 0, 0}, o_scratch = 0,
            o_pos = 0, o_tile_ptr = 0, o_tile_frames = 0, o_partials = 0, o_err_partials = 0, o_err_sums = 0, o_pnum = 0,
            o_pden = 0, o_scalars = 0, o_total = 0;
 
@@ -243,6 +243,7 @@ OverlapArgs base_overlap_args(sharp_plan_t *p)
     a.tile_ptr = p->dp<int>(p->o_tile_ptr);
     a.tile_frames = p->dp<int>(p->o_tile_frames);
     a.den = p->dp<float>(p->o_den);
+    a.cross = p->dp<float2>(p->o_cross);
     return a;
 }
 
@@ -303,6 +304,8 @@ int rebuild_den(sharp_plan_t *p)
 {
     OverlapArgs a = base_overlap_args(p);
     a.w_a = p->dp<float2>(p->o_w[p->w_cur]);
+    // the frames may have been formed with another probe: keep sum conj(w_cur) w_form for the re-gather
+    a.w_b = (p->have_frames && !p->psi_v_zero) ? p->dp<float2>(p->o_w[p->w_form]) : nullptr;
     return overlap_launch<OV_DEN>(p, a);
 }
 
@@ -413,6 +416,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->o_psi_v[0] = take(p->nobj() * 8);
     p->o_psi_v[1] = take(p->nobj() * 8);
     p->o_den = take(p->nobj() * 4);
+    p->o_cross = take(p->nobj() * 8);
     for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
     // m <= 128 keeps the frame in shared memory; above, one L2 scratch slot per cluster of CTAs
     const int cs_plan = m == 256 ? kCluster256 : kCluster512;
