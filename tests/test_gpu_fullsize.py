@@ -86,3 +86,39 @@ def test_config4_size_sampled_operators(oracle):
         want = np.sum(np.conj(wv) * fv) / den
         assert abs(complex(psi[pr, pc]) - want) <= 2e-5 * max(abs(want), np.sqrt(np.sum(np.abs(fv) ** 2) / den) * 1e-1), (pr, pc)
     rec.close()
+
+
+def test_config3_full_one_blind_iteration(oracle):
+    """The blind loop at full config-3 size: RAAR step, Eq. 9, Eq. 10, Q*Q + cross rebuild and re-gather, once,
+    teacher-forced from a GPU state (reading G10 order).  The probe update divides by sum |psi|^2 and psi itself is
+    a ratio at weakly lit pixels, so the bar is the oracle's own sensitivity to a 1e-7 input perturbation (x10),
+    floored at the operator tolerance, as in test_probe_refinement_sequence_G10."""
+    cfg = synth.config(3)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    rec = sharp.Reconstruction(cfg.m, pos, shape)
+    rec.set_intensities(I); rec.set_probe(w0); rec.set_object(None)
+    rec.set_probe_refine(0)
+    rec.iterate(2, cfg.beta)                       # fixed-probe warm-up to a generic state
+    z = rec.get_frames().cpu().numpy()
+    rec.set_probe_refine(1)
+    rec.iterate(1, cfg.beta)
+    z1 = rec.get_frames().cpu().numpy()
+    w1 = rec.get_probe().cpu().numpy()
+    o = oracle.Oracle(cfg.m, pos, shape, I, w0, refine_every=1)
+    o.set_frames(z)
+    o.it = 0
+    o.iterate(1, cfg.beta)
+    rng = np.random.default_rng(5)
+    o2 = oracle.Oracle(cfg.m, pos, shape, I, w0, refine_every=1)
+    o2.set_frames((z * (1 + 1e-7 * rng.standard_normal(z.shape))).astype(np.complex64))
+    o2.iterate(1, cfg.beta)
+    assert rel(z1, o.z) < 1e-5
+    tol_w = max(2e-5, 10 * rel(o2.w, o.w))
+    assert rel(w1, o.w) < tol_w, (rel(w1, o.w), tol_w)
+    psi = rec.get_object().cpu().numpy()
+    den = oracle.overlap_den(o.w, pos, shape)
+    lit = den >= 1e-3 * den.max()
+    want_psi = o.object()
+    tol_p = max(5e-5, 10 * rel(o2.object()[lit], want_psi[lit]))
+    assert rel(psi[lit], want_psi[lit]) < tol_p
+    rec.close()

@@ -307,3 +307,40 @@ def test_tma_overlap_path(oracle, monkeypatch):
     want2 = oracle.raar(oracle.raar(z, wt, pos, shape, a, thr, cfg.beta), wt, pos, shape, a, thr, cfg.beta)
     assert rel(rec.get_frames().cpu().numpy(), want2) < 3 * OP_TOL
     rec.close()
+
+
+@pytest.mark.parametrize("n", [2, 4])
+def test_bitwise_determinism(n):
+    """No float atomics and a fixed summation order (reading G17): two runs give bit-identical frames, object and
+    residuals, also with the probe refined."""
+    cfg = synth.reduced(synth.config(n), 5)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    outs = []
+    for _ in range(2):
+        rec = sharp.Reconstruction(cfg.m, pos, shape)
+        rec.set_intensities(I); rec.set_probe(w0); rec.set_object(None)
+        rec.set_probe_refine(2)
+        rec.iterate(7, cfg.beta)
+        outs.append((rec.get_frames().cpu().numpy(), rec.get_object().cpu().numpy(), rec.get_probe().cpu().numpy(),
+                     rec.errors()))
+        rec.close()
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a.view(np.uint8) if a.dtype != np.float64 else a, b.view(np.uint8) if b.dtype != np.float64 else b)
+
+
+def test_profile_hooks():
+    cfg = synth.reduced(synth.config(1), 4)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    rec = sharp.Reconstruction(cfg.m, pos, shape)
+    rec.set_intensities(I); rec.set_probe(w0); rec.set_object(None)
+    rec.profile(True)
+    l0 = rec.launch_count()
+    rec.iterate(5, cfg.beta)
+    p = rec.profile_read()
+    assert p["frame"][1] == 5 and p["overlap"][1] == 5 and p["probe"][1] == 0
+    assert p["frame"][0] > 0 and p["overlap"][0] > 0
+    assert rec.launch_count() - l0 == 10           # exactly two kernels per RAAR iteration
+    rec.profile(False)
+    rec.iterate(1, cfg.beta)
+    assert rec.profile_read()["frame"][1] == 0
+    rec.close()
