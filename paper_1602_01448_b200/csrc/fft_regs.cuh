@@ -26,8 +26,30 @@ SHARP_HD constexpr float w32_cos(int e)
 }
 SHARP_HD constexpr float w32_sin(int e) { return w32_cos(e - 8); }
 
-SHARP_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-SHARP_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Complex add / subtract as ONE packed instruction on sm_100a (add.f32x2 / sub.f32x2 -> FADD2): the butterflies are
+// mostly these, and the passes are issue-slot bound, so halving their instruction count matters; each component is
+// still one IEEE round-to-nearest add (the only numerical difference to the scalar form is that the compiler can no
+// longer contract such an add with a neighbouring multiply into an FMA).
+SHARP_HD float2 cadd(float2 a, float2 b)
+{
+#if defined(__CUDA_ARCH__) && __CUDA_ARCH__ >= 1000 && !defined(SHARP_NO_PACKED_F32)
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long *>(&a)), "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+#else
+    return make_float2(a.x + b.x, a.y + b.y);
+#endif
+}
+SHARP_HD float2 csub(float2 a, float2 b)
+{
+#if defined(__CUDA_ARCH__) && __CUDA_ARCH__ >= 1000 && !defined(SHARP_NO_PACKED_F32)
+    unsigned long long d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long *>(&a)), "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+#else
+    return make_float2(a.x - b.x, a.y - b.y);
+#endif
+}
 SHARP_HD float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 // a * conj(b)
 SHARP_HD float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }
