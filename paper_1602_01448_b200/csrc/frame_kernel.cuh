@@ -53,7 +53,6 @@ struct FrameArgs {
     float bm;                // beta / m^2
     float om;                // 1 - 2 beta
     int conj_io;             // FRAME_FFT: conjugate input and output (gives F*)
-    int stagger_ns;          // k_frame_ws128: delay of consumer group 1 at every stage start (phase staggering)
     // FRAME_ERR only
     const float2 *c_prev, *psi_v_prev, *w_form_prev;   // previous iterate in factored form (c_prev NULL: z_prev = 0)
     const float2 *psi_z, *w_cur;                        // P_Q z = w_cur . T psi_z

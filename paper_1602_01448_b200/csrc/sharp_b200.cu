@@ -65,7 +65,6 @@ struct sharp_plan_s {
     bool prev_psi_v_zero = true;
     int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
     int refine_every = 0;
-    int stagger_ns = 0;                // SHARP_WS_STAGGER_NS: see FrameArgs::stagger_ns
     bool use_tma_overlap = false;      // SHARP_OVERLAP_TMA=1 selects the TMA-box overlap (slower in round 1: w is not L1-cached)
     bool use_ws = true;                // m = 128: warp-specialised iteration kernel (SHARP_FRAME_WS=0 disables)
     long long it = 0;
@@ -230,7 +229,6 @@ FrameArgs base_frame_args(sharp_plan_t *p)
     a.sc = p->dp<DevScalars>(p->o_scalars);
     a.K = p->K;
     a.nc = p->nc;
-    a.stagger_ns = p->stagger_ns;
     return a;
 }
 
@@ -374,7 +372,6 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->m = m; p->K = K; p->nr = obj_rows; p->nc = obj_cols;
     p->E = (m == 512) ? 32 : 16;
     p->use_ws = env_int("SHARP_FRAME_WS", 1) != 0;
-    p->stagger_ns = env_int("SHARP_WS_STAGGER_NS", 0);
     p->use_tma_overlap = env_int("SHARP_OVERLAP_TMA", 0) != 0;
     p->pos.assign(pos_rc, pos_rc + 2 * (size_t)K);
     p->tiles_r = (obj_rows + TILE - 1) / TILE;
