@@ -132,7 +132,7 @@ __device__ __forceinline__ void cluster_barrier()
 
 // Launched with cluster dimension CS (CS = 1: plain launch).  gridDim.x is a multiple of CS.
 template <int M, int E, int NT, int MODE, int CS>
-__global__ void __launch_bounds__(NT, (E <= 16 ? 2 : 1)) k_frame(FrameArgs A)
+__global__ void __launch_bounds__(NT, 2) k_frame(FrameArgs A)
 {
     using C = FrameCfg<M, E, NT>;
     constexpr int TPL = C::TPL, L = C::L, RB = C::RB;
