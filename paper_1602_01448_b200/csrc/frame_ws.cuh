@@ -6,7 +6,9 @@
 //
 //   * one PRODUCER warpgroup (4 warps) stages z = c + w_form . T psi_v for the rows of the NEXT frame: the state c
 //     goes straight from global into the staging slot with cp.async (16-byte copies, no registers, all four rows
-//     of a warp in flight), the probe and the object tile come through registers with coalesced 128/64-bit loads,
+//     of a warp in flight), the object tile comes through registers with coalesced 64-bit loads, the probe is parked
+//     once per launch in the producer threads' own TMEM lanes (128 KB of the SM's 256 KB tensor memory) and read
+//     back with tcgen05.ld, so it costs L2 -> SM bandwidth once per launch instead of once per frame,
 //     and each thread then combines in place the locations it copied itself.  Six 16-row chunks go to a ring in
 //     shared memory (96 KB, one full/empty mbarrier pair per slot), the last two (rows 96..127) in place into the
 //     frame buffer once the consumers have retired those rows, so a whole frame is staged ahead and none of the
@@ -35,7 +37,7 @@ struct WsCfg {
     static constexpr int NCONS = 512, NPROD = 128, NT = NCONS + NPROD, GSZ = 256, L = 32;  // L: lines per group pass
     static constexpr int SR = 16, NSLOT = 6, CHUNKS = M / SR;                                // ring geometry
     static constexpr int F_BYTES = M * M * 8, S_BYTES = NSLOT * SR * M * 8;
-    static constexpr int SMEM_BYTES = F_BYTES + S_BYTES + (2 * NSLOT + 3) * 8;
+    static constexpr int SMEM_BYTES = F_BYTES + S_BYTES + (2 * NSLOT + 3) * 8 + 8;   // + TMEM base slot
     static constexpr int REGS_LAUNCH = 96;   // 640 threads x 96 registers = 61440 of the SM's 65536
 };
 
@@ -77,6 +79,37 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+// Tensor memory (TMEM, 256 KB per SM, otherwise idle in this kernel) as a register-file extension of the producer:
+// a thread's probe values are the same for every frame, so they are parked once per launch in the thread's own
+// TMEM lane (32 rows x 4 pixels x 8 bytes = 256 columns) and read back with tcgen05.ld when a chunk is combined.
+__device__ __forceinline__ void tmem_alloc_256(unsigned *smem_slot)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" ::"r"(smem_u32(smem_slot)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_256(unsigned taddr)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(unsigned taddr, const float4 &a, const float4 &b)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+                 "r"(__float_as_uint(a.x)), "r"(__float_as_uint(a.y)), "r"(__float_as_uint(a.z)), "r"(__float_as_uint(a.w)),
+                 "r"(__float_as_uint(b.x)), "r"(__float_as_uint(b.y)), "r"(__float_as_uint(b.z)), "r"(__float_as_uint(b.w))
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(unsigned taddr, float4 &a, float4 &b)
+{
+    unsigned r0, r1, r2, r3, r4, r5, r6, r7;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3), "=r"(r4), "=r"(r5), "=r"(r6), "=r"(r7)
+                 : "r"(taddr)
+                 : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    a = make_float4(__uint_as_float(r0), __uint_as_float(r1), __uint_as_float(r2), __uint_as_float(r3));
+    b = make_float4(__uint_as_float(r4), __uint_as_float(r5), __uint_as_float(r6), __uint_as_float(r7));
+}
+
 // production order of the eight 16-row chunks of a frame: position j -> chunk q, and its inverse
 __device__ __forceinline__ int ws_chunk_of(int j) { return (j & 1) | ((j & 2) << 1) | ((j & 4) >> 1); }
 __device__ __forceinline__ int ws_seq_of(int q) { return (q & 1) | ((q & 4) >> 1) | ((q & 2) << 1); }
@@ -92,6 +125,7 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
     unsigned long long *empty = full + NSLOT;
     unsigned long long *fullF = empty + NSLOT;   // [2]: chunks 6, 7 are produced in place in F rows 96..127
     unsigned long long *emptyF = fullF + 2;      // group 1 has retired F rows 96..127 (8 warp arrivals)
+    unsigned *tmem_slot = reinterpret_cast<unsigned *>(emptyF + 1);
 
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -112,6 +146,23 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
         if (pw == 0 && lane == 0 && (int)blockIdx.x < A.K) {
             prefetch_l2_bulk(A.c_in + (size_t)blockIdx.x * M * M, M * M * 8);
             prefetch_l2_bulk(A.a_int + (size_t)blockIdx.x * M * M, M * M * 4);
+        }
+        // probe -> TMEM, once per launch (lanes 32 pw .. 32 pw + 31 belong to this warp)
+        const bool w_tmem = A.psi_v != nullptr;
+        unsigned tw_addr = 0;
+        if (w_tmem) {
+            if (pw == 0) tmem_alloc_256(tmem_slot);
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            named_bar_sync(4, C::NPROD);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            tw_addr = *reinterpret_cast<volatile unsigned *>(tmem_slot) + ((unsigned)(32 * pw) << 16);
+#pragma unroll 1
+            for (int qr = 0; qr < 32; ++qr) {   // qr = 4 q + rr
+                const int r = (qr >> 2) * SR + 4 * pw + (qr & 3);
+                const float4 *w4 = reinterpret_cast<const float4 *>(A.w_form + r * M);
+                tmem_st8(tw_addr + 8 * qr, __ldg(w4 + lane), __ldg(w4 + 32 + lane));
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         }
         int fseq = 0;  // frames this CTA has staged
         for (int i = blockIdx.x; i < A.K; i += gridDim.x, ++fseq) {
@@ -150,15 +201,14 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
 #pragma unroll
                     for (int rr = 0; rr < 4; ++rr) {
                         const int r = q * SR + 4 * pw + rr;
-                        const float4 *w4 = reinterpret_cast<const float4 *>(A.w_form + r * M);
-                        wv[rr][0] = __ldg(w4 + lane);
-                        wv[rr][1] = __ldg(w4 + 32 + lane);
                         const float2 *prow = A.psi_v + (size_t)(xr + r) * A.nc + xc;
                         pv[rr][0] = __ldg(prow + 2 * lane);
                         pv[rr][1] = __ldg(prow + 2 * lane + 1);
                         pv[rr][2] = __ldg(prow + 64 + 2 * lane);
                         pv[rr][3] = __ldg(prow + 64 + 2 * lane + 1);
                     }
+#pragma unroll
+                    for (int rr = 0; rr < 4; ++rr) tmem_ld8(tw_addr + 8 * (4 * q + rr), wv[rr][0], wv[rr][1]);
                     cp_async_wait_all();
 #pragma unroll
                     for (int rr = 0; rr < 4; ++rr) {
@@ -181,6 +231,11 @@ __global__ void __launch_bounds__(WsCfg::NT, 1) k_frame_ws128(FrameArgs A)
                 }
                 mbar_arrive(inF ? fullF + (j - NSLOT) : full + j);
             }
+        }
+        if (w_tmem) {
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            named_bar_sync(4, C::NPROD);
+            if (pw == 0) tmem_dealloc_256(*reinterpret_cast<volatile unsigned *>(tmem_slot));
         }
         return;
     }
