@@ -57,7 +57,7 @@ def parse():
 
 
 def workload(args, rank=0):
-    from paper_1602_01448_b200 import synth
+    import synth
     cfg = synth.config(args.config)
     if args.grid:
         cfg = synth.reduced(cfg, args.grid)
@@ -77,7 +77,7 @@ def workload_name(cfg, iters):
 # ---- the CPU oracle, timed as it stands (cpu_baseline and --impl reference) ---------------------------------------
 def oracle_sample(args):
     """A sub-raster of the same recipe that the oracle advances in a few seconds per step."""
-    from paper_1602_01448_b200 import synth
+    import synth
     cfg = synth.config(args.config)
     g = {64: 10, 128: 12, 256: 6, 512: 9}[cfg.m]          # frames: 100 / 144 / 36 / 9
     scfg = synth.reduced(cfg, min(g, cfg.grid))
@@ -86,7 +86,7 @@ def oracle_sample(args):
 
 
 def time_oracle(args, steps, warmup):
-    from paper_1602_01448_b200 import synth
+    import synth
     from oracle import sharp_oracle as orc
     orc.build()
     scfg, its = oracle_sample(args)
@@ -205,7 +205,7 @@ def job_value(world, K, iters, steps, ms):
 def run_ours(args):
     import torch
     import paper_1602_01448_b200 as sharp
-    from paper_1602_01448_b200 import synth
+    import synth
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -82,6 +82,10 @@ int sharp_set_object(sharp_plan_t *p, const float *psi_dev);
 /* sharp_set_frames: z_dev is DEVICE, K*m*m c64.  Overwrites the frame state (restore / teacher forcing);
  * the "previous iterate" of eps_Delta becomes 0 as before the first iteration. Needs the probe. */
 int sharp_set_frames(sharp_plan_t *p, const float *z_dev);
+/* sharp_set_frame_slots: caps the number of frames the fused per-frame kernel keeps in flight (persistent CTAs at
+ * m <= 128, CTA clusters above); 0 = one per resident slot of the bound device (the default).  A tuning and test
+ * hook: with fewer slots than frames every CTA loops over several frames. May be called before or after sharp_bind. */
+int sharp_set_frame_slots(sharp_plan_t *p, int slots);
 /* Illumination refinement every `every` iterations (Eq. 10; PAPER.md:181 "if desired", :228); 0 = fixed probe. */
 int sharp_set_probe_refine(sharp_plan_t *p, int every);
 

@@ -31,6 +31,7 @@ _SIGNATURES = {
     "sharp_set_object": (_i, [_vp, _vp]),
     "sharp_set_frames": (_i, [_vp, _vp]),
     "sharp_set_probe_refine": (_i, [_vp, _i]),
+    "sharp_set_frame_slots": (_i, [_vp, _i]),
     "sharp_iterate": (_i, [_vp, _i, _f]),
     "sharp_get_object": (_i, [_vp, _vp]),
     "sharp_get_probe": (_i, [_vp, _vp]),
@@ -178,6 +179,9 @@ class Reconstruction:
 
     def set_probe_refine(self, every):
         self._check(self.lib.sharp_set_probe_refine(self._plan, int(every)))
+
+    def set_frame_slots(self, slots):
+        self._check(self.lib.sharp_set_frame_slots(self._plan, int(slots)))
 
     def iterate(self, n, beta):
         self._check(self.lib.sharp_iterate(self._plan, int(n), float(beta)))

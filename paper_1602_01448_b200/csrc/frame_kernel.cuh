@@ -25,39 +25,9 @@
 // Shared strip layout: element (line, pos) at line * M + (pos ^ (bitrev3(line & 7) << 1)).
 #pragma once
 #include "fft_regs.cuh"
+#include "frame_common.cuh"
 
 namespace sharp {
-
-enum FrameMode : int {
-    FRAME_ITER = 0,  // c_out = beta z + (1-2 beta) P_a z
-    FRAME_FFT = 1,   // c_out = F z  in natural (u,v) order, unitary (test hook)
-    FRAME_ERR = 2    // no output; accumulates ||P_a z - z||^2, ||P_Q z - z||^2, ||z - z_prev||^2
-};
-
-struct DevScalars {
-    double A2;       // ||a||^2 = sum I          (reading G12)
-    float thr2;      // (m * thr)^2, thr = 1e-4 a_rms: threshold on |Z^|^2 (reading G4)
-    float pad;
-};
-
-struct FrameArgs {
-    const float2 *c_in;      // K m m   frame-local state (or the operand of the op_* hooks)
-    float2 *c_out;           // K m m
-    const float *a_int;      // K m m   amplitudes / m in position space
-    const float2 *psi_v;     // object; may be NULL (z = c_in)
-    const float2 *w_form;    // m m
-    const int *pos;          // K x 2
-    float2 *scratch;         // gridDim.x * m * m
-    const DevScalars *sc;
-    int K, nc;
-    float bm;                // beta / m^2
-    float om;                // 1 - 2 beta
-    int conj_io;             // FRAME_FFT: conjugate input and output (gives F*)
-    // FRAME_ERR only
-    const float2 *c_prev, *psi_v_prev, *w_form_prev;   // previous iterate in factored form (c_prev NULL: z_prev = 0)
-    const float2 *psi_z, *w_cur;                        // P_Q z = w_cur . T psi_z
-    double *err_partials;                               // gridDim.x * 3
-};
 
 template <int M, int E, int NT>
 struct FrameCfg {
@@ -68,11 +38,6 @@ struct FrameCfg {
 };
 
 __device__ __forceinline__ int swz(int line, int pos) { return pos ^ ((__brev((unsigned)(line & 7)) >> 29) << 1); }
-
-__device__ __forceinline__ float2 ld_stream(const float2 *p) { return __ldcs(p); }
-__device__ __forceinline__ void st_stream(float2 *p, float2 v) { __stcs(p, v); }
-__device__ __forceinline__ float2 ld_l2(const float2 *p) { return __ldcg(p); }
-__device__ __forceinline__ void st_l2(float2 *p, float2 v) { __stcg(p, v); }
 
 // A-side twiddles W_M^{k s} (k < E), conjugated for the inverse.  E == 16: per-thread registers; otherwise a
 // shared table of M entries.
@@ -114,20 +79,6 @@ __device__ __forceinline__ void dft_b(float2 *v)
 {
 #pragma unroll
     for (int q = 0; q < E / RB; ++q) dft<RB, SGN>(v + q * RB);
-}
-
-// Cluster helpers: the CS CTAs of a thread-block cluster share one frame (and one L2 scratch slot); strips are
-// dealt round-robin by cluster rank and the three stage changes are cluster barriers (release/acquire, so the
-// L2-resident scratch written with st.cg by one CTA is visible to the ld.cg of the others).
-__device__ __forceinline__ unsigned cluster_rank()
-{
-    unsigned r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void cluster_barrier()
-{
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
 // Launched with cluster dimension CS (CS = 1: plain launch).  gridDim.x is a multiple of CS.

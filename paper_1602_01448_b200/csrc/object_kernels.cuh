@@ -3,6 +3,7 @@
 // amplitude preparation (a0) and small helpers.
 #pragma once
 #include "frame_kernel.cuh"
+#include "frame_r.cuh"
 
 namespace sharp {
 
@@ -66,24 +67,34 @@ __global__ void __launch_bounds__(256) k_frame_index(int m, int K, const int *po
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// a0 amplitudes:  a = sqrt(max(I, 0))  (reading G14), stored as a/m in the FFT's position space:
-//     a_int[i][q][p] = a[i][freq(q)][freq(p)] / m,   freq(x) = x / RB + RA (x % RB).
+// a0 amplitudes:  a = sqrt(max(I, 0))  (reading G14), stored as a/m in the order in which the frame
+// kernel of this frame size meets the Fourier coefficients ("slots"): slot_freq() of frame_r.cuh for m <= 128,
+// the position space of frame_kernel.cuh (freq(x) = x / RB + RA (x % RB) on both axes) above.
 // Also per-block partial sums of max(I,0) in double (||a||^2, reading G12); k_scalars finishes them in a fixed
-// order.  natural != 0 is the inverse map (a_int -> a, for sharp_get_amplitudes).
+// order.  k_amplitudes_natural is the inverse map (a_int -> a, for sharp_get_amplitudes).
 // ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void amp_slot_freq(int m, int RA, int slot, int &u, int &v)
+{
+    if (m == 64) slot_freq<64>(slot, u, v);
+    else if (m == 128) slot_freq<128>(slot, u, v);
+    else {
+        const int RB = m / RA, q = slot / m, p = slot % m;
+        u = q / RB + RA * (q % RB);
+        v = p / RB + RA * (p % RB);
+    }
+}
+
 __global__ void __launch_bounds__(256) k_amplitudes(int m, int RA, int K, const float *I, float *a_int,
                                                      double *partials)
 {
-    const int RB = m / RA;
     const size_t per_frame = (size_t)m * m;
     const size_t total = (size_t)K * per_frame;
     const float inv_m = 1.0f / (float)m;
     double acc = 0.0;
     for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
         const size_t i = g / per_frame;
-        const size_t rem = g - i * per_frame;
-        const int q = (int)(rem / m), p = (int)(rem % m);
-        const int u = q / RB + RA * (q % RB), v = p / RB + RA * (p % RB);
+        int u, v;
+        amp_slot_freq(m, RA, (int)(g - i * per_frame), u, v);
         const float val = fmaxf(__ldg(I + i * per_frame + (size_t)u * m + v), 0.0f);
         acc += (double)val;
         a_int[g] = sqrtf(val) * inv_m;
@@ -100,14 +111,12 @@ __global__ void __launch_bounds__(256) k_amplitudes(int m, int RA, int K, const 
 
 __global__ void k_amplitudes_natural(int m, int RA, int K, const float *a_int, float *a)
 {
-    const int RB = m / RA;
     const size_t per_frame = (size_t)m * m;
     const size_t total = (size_t)K * per_frame;
     for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
         const size_t i = g / per_frame;
-        const size_t rem = g - i * per_frame;
-        const int q = (int)(rem / m), p = (int)(rem % m);
-        const int u = q / RB + RA * (q % RB), v = p / RB + RA * (p % RB);
+        int u, v;
+        amp_slot_freq(m, RA, (int)(g - i * per_frame), u, v);
         a[i * per_frame + (size_t)u * m + v] = a_int[g] * (float)m;
     }
 }

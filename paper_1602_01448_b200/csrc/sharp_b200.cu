@@ -12,24 +12,20 @@
 #include <string>
 #include <vector>
 
-#include "frame_ws.cuh"
+#include "frame_kernel.cuh"
+#include "frame_r.cuh"
 #include "object_kernels.cuh"
-#include "overlap_tma.cuh"
 
 using namespace sharp;
 
 namespace {
 
 constexpr double kTau = 1e-4;  // reading G4: thr = tau * a_rms
+constexpr int kMaxFrameSlots = 1024;   // upper bound on the persistent frame grid (sizes the error partials)
+constexpr int kMaxScratchCtas = 2 * 160;  // m >= 256: CTAs whose clusters own an L2 scratch slot
 thread_local std::string g_plan_error = "";
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
-
-int env_int(const char *name, int dflt)
-{
-    const char *s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
 
 }  // namespace
 
@@ -49,6 +45,10 @@ struct sharp_plan_s {
     size_t ws_bytes = 0;
     int frame_grid = 0;      // persistent CTAs of the frame kernel
     int slots_cap = 0;       // upper bound on frame_grid the workspace was sized for
+    int slots_user = 0;      // sharp_set_frame_slots: caps the persistent grid (0 = one CTA per SM slot)
+    int sms = 0;             // multiprocessors of the bound device
+    int device = -1;         // CUDA device the plan was bound on
+    int frame_ctas_max = 0;  // resident CTAs of the iteration kernel on that device
     int frame_nt = 256;
     int probe_chunk = 64, probe_nchunks = 0;
     int amp_blocks = 0;
@@ -65,8 +65,6 @@ struct sharp_plan_s {
     bool prev_psi_v_zero = true;
     int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
     int refine_every = 0;
-    bool use_tma_overlap = false;      // SHARP_OVERLAP_TMA=1 selects the TMA-box overlap (slower in round 1: w is not L1-cached)
-    bool use_ws = true;                // m = 128: warp-specialised iteration kernel (SHARP_FRAME_WS=0 disables)
     long long it = 0;
     long long launches = 0;
 
@@ -129,15 +127,15 @@ struct ProfScope {
     ~ProfScope() { if (end) cudaEventRecord(end, p->stream); }
 };
 
-int grid_for(size_t n, int per_block = 256, int cap = 148 * 16)
+int grid_for(size_t n, int per_block = 256, int cap = 160 * 16)
 {
     size_t b = (n + per_block - 1) / per_block;
     return (int)std::min<size_t>(std::max<size_t>(b, 1), (size_t)cap);
 }
 
 // ---- frame kernel dispatch -----------------------------------------------------------------------------------
-// m = 64, 128: the frame lives in shared memory (frame_smem.cuh).  m = 256, 512: strips in shared memory, the
-// row<->column transposition through a per-CTA scratch in L2 (frame_kernel.cuh).
+// m = 64, 128: the register-radix kernel of frame_r.cuh (whole frame on one SM).  m = 256, 512: strips in shared
+// memory, the row<->column transposition through a per-cluster scratch in L2 (frame_kernel.cuh).
 template <int M, int E, int NT, int MODE>
 int frame_smem_bytes()
 {
@@ -153,8 +151,7 @@ cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int *blocks_per_sm)
 }
 
 // m >= 256: CS CTAs of a cluster share one frame, so that the scratch slots in flight (one per cluster) stay
-// inside L2: 148 x 512 KB at m = 256, 18 x 2 MB at m = 512.  Measured at m = 256 (1,600 frames): 1 CTA per frame (296
-// slots, 155 MB: spills) 1.40 ms, clusters of 2 1.16 ms, clusters of 4 1.70 ms (barrier cost and imbalance).
+// inside L2: 148 x 512 KB at m = 256, 18 x 2 MB at m = 512.
 constexpr int kCluster256 = 2, kCluster512 = 8;
 
 template <class KernelT>
@@ -181,13 +178,8 @@ int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
 {
     ProfScope prof(p, MODE == FRAME_ITER ? SHARP_PROF_FRAME : SHARP_PROF_OTHER);
     switch (p->m) {
-    case 64: k_frame_smem<64, 256, MODE><<<grid, 256, SmemFrameCfg<64, 256>::SMEM_BYTES, p->stream>>>(a); break;
-    case 128:
-        if (MODE == FRAME_ITER && p->use_ws)
-            k_frame_ws128<<<grid, WsCfg::NT, WsCfg::SMEM_BYTES, p->stream>>>(a);
-        else
-            k_frame_smem<128, 512, MODE><<<grid, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, p->stream>>>(a);
-        break;
+    case 64: k_frame_r<64, MODE><<<grid, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, p->stream>>>(a); break;
+    case 128: k_frame_r<128, MODE><<<grid, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, p->stream>>>(a); break;
     case 256:
         CK(launch_cluster(k_frame<256, 16, 256, MODE, kCluster256>, grid, 256, frame_smem_bytes<256, 16, 256, MODE>(),
                           kCluster256, p->stream, a));
@@ -206,14 +198,8 @@ template <int MODE>
 cudaError_t frame_prepare_m(int m, int *bps)
 {
     switch (m) {
-    case 64: return kernel_prepare(k_frame_smem<64, 256, MODE>, 256, SmemFrameCfg<64, 256>::SMEM_BYTES, bps);
-    case 128: {
-        if (MODE == FRAME_ITER) {
-            cudaError_t e = kernel_prepare(k_frame_ws128, WsCfg::NT, WsCfg::SMEM_BYTES, bps);
-            if (e != cudaSuccess) return e;
-        }
-        return kernel_prepare(k_frame_smem<128, 512, MODE>, 512, SmemFrameCfg<128, 512>::SMEM_BYTES, bps);
-    }
+    case 64: return kernel_prepare(k_frame_r<64, MODE>, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, bps);
+    case 128: return kernel_prepare(k_frame_r<128, MODE>, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, bps);
     case 256: return kernel_prepare(k_frame<256, 16, 256, MODE, kCluster256>, 256, frame_smem_bytes<256, 16, 256, MODE>(), bps);
     default: return kernel_prepare(k_frame<512, 32, 256, MODE, kCluster512>, 256, frame_smem_bytes<512, 32, 256, MODE>(), bps);
     }
@@ -245,54 +231,10 @@ OverlapArgs base_overlap_args(sharp_plan_t *p)
     return a;
 }
 
-// ---- tensor maps for the TMA overlap (driver entry point resolved at run time: no link dependency on libcuda) ----
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_tiled_fn()
-{
-    static EncodeTiledFn fn = [] {
-        void *ptr = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) != cudaSuccess ||
-            q != cudaDriverEntryPointSuccess)
-            ptr = nullptr;
-        return reinterpret_cast<EncodeTiledFn>(ptr);
-    }();
-    return fn;
-}
-
-// rank-3 map over K frames of m x m c64 (8-byte elements), or rank-2 over one m x m array; box TILE x TILE (x 1),
-// out-of-range coordinates read as zero.
-bool make_box_map(CUtensorMap *map, const void *base, int m, long long K)
-{
-    EncodeTiledFn enc = encode_tiled_fn();
-    if (!enc) return false;
-    const cuuint32_t rank = K > 0 ? 3 : 2;
-    cuuint64_t dims[3] = {(cuuint64_t)m, (cuuint64_t)m, (cuuint64_t)(K > 0 ? K : 1)};
-    cuuint64_t strides[2] = {(cuuint64_t)m * 8, (cuuint64_t)m * m * 8};
-    cuuint32_t box[3] = {OVT_BOXW, TILE, 1};
-    cuuint32_t estr[3] = {1, 1, 1};
-    return enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, rank, const_cast<void *>(base), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 template <int MODE>
 int overlap_launch(sharp_plan_t *p, const OverlapArgs &a)
 {
     ProfScope prof(p, MODE == OV_ITER ? SHARP_PROF_OVERLAP : SHARP_PROF_OTHER);
-    if constexpr (MODE == OV_ITER || MODE == OV_L) {
-        if (p->use_tma_overlap) {
-            CUtensorMap mf, mw;
-            if (!make_box_map(&mf, a.f, p->m, p->K) || !make_box_map(&mw, a.w_a, p->m, 0))
-                return fail(p, SHARP_ECUDA, "cuTensorMapEncodeTiled failed");
-            k_overlap_tma<MODE><<<p->tiles_r * p->tiles_c, 256, OVT_SMEM_BYTES, p->stream>>>(a, mf, mw);
-            CK_LAUNCH("k_overlap_tma");
-            return SHARP_OK;
-        }
-    }
     k_overlap<MODE><<<p->tiles_r * p->tiles_c, 256, 0, p->stream>>>(a);
     CK_LAUNCH("k_overlap");
     return SHARP_OK;
@@ -317,6 +259,18 @@ int regather_psi_z(sharp_plan_t *p)
     a.psi_z = p->dp<float2>(p->o_psi_z);
     a.psi_v_in = p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]);
     return overlap_launch<OV_REGATHER>(p, a);
+}
+
+// persistent grid of the frame kernels: one CTA (m <= 128) or one cluster (m >= 256) per resident slot, never more
+// than there are frames; sharp_set_frame_slots lowers it (tests force several rounds per CTA that way)
+void update_frame_grid(sharp_plan_t *p)
+{
+    const int cs = p->m <= 128 ? 1 : (p->m == 256 ? kCluster256 : kCluster512);
+    long long units = std::min<long long>(p->K, p->frame_ctas_max / cs);
+    if (cs > 1) units = std::min<long long>(units, kMaxScratchCtas / cs);
+    units = std::min<long long>(units, kMaxFrameSlots / cs);
+    if (p->slots_user > 0) units = std::min<long long>(units, p->slots_user);
+    p->frame_grid = (int)std::max<long long>(1, units) * cs;
 }
 
 int free_probe_slot(const sharp_plan_t *p)
@@ -371,8 +325,6 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     if (!p) return fail(nullptr, SHARP_ENOMEM, "host allocation failed");
     p->m = m; p->K = K; p->nr = obj_rows; p->nc = obj_cols;
     p->E = (m == 512) ? 32 : 16;
-    p->use_ws = env_int("SHARP_FRAME_WS", 1) != 0;
-    p->use_tma_overlap = env_int("SHARP_OVERLAP_TMA", 0) != 0;
     p->pos.assign(pos_rc, pos_rc + 2 * (size_t)K);
     p->tiles_r = (obj_rows + TILE - 1) / TILE;
     p->tiles_c = (obj_cols + TILE - 1) / TILE;
@@ -398,10 +350,9 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     }
 
     // workspace layout.  The frame kernel is persistent: at most one scratch slot per resident CTA.
-    const int slots_cap = std::max(1, env_int("SHARP_FRAME_SLOTS", 148 * 2));
+    const int slots_cap = kMaxFrameSlots;
     p->slots_cap = slots_cap;
-    p->frame_grid = std::min(K, slots_cap);
-    p->probe_chunk = std::max(1, env_int("SHARP_PROBE_CHUNK", 32));
+    p->probe_chunk = 32;
     p->probe_nchunks = (K + p->probe_chunk - 1) / p->probe_chunk;
     p->amp_blocks = grid_for(p->npx());
     size_t o = 0;
@@ -417,7 +368,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
     // m <= 128 keeps the frame in shared memory; above, one L2 scratch slot per cluster of CTAs
     const int cs_plan = m == 256 ? kCluster256 : kCluster512;
-    p->o_scratch = take(m <= 128 ? 256 : (size_t)((slots_cap + cs_plan - 1) / cs_plan) * m * m * 8);
+    p->o_scratch = take(m <= 128 ? 256 : (size_t)std::min(K, kMaxScratchCtas / cs_plan) * m * m * 8);
     p->o_pos = take((size_t)K * 2 * 4);
     p->o_tile_ptr = take((ntiles + 1) * 4);
     p->o_tile_frames = take(std::max<size_t>(p->tile_frames.size(), 1) * 4);
@@ -461,22 +412,14 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     int bps2 = 0;
     CK(frame_prepare_m<FRAME_FFT>(p->m, &bps2));
     CK(frame_prepare_m<FRAME_ERR>(p->m, &bps2));
-    CK(cudaFuncSetAttribute(k_overlap_tma<OV_ITER>, cudaFuncAttributeMaxDynamicSharedMemorySize, OVT_SMEM_BYTES));
-    CK(cudaFuncSetAttribute(k_overlap_tma<OV_L>, cudaFuncAttributeMaxDynamicSharedMemorySize, OVT_SMEM_BYTES));
-    if (p->use_tma_overlap && !encode_tiled_fn()) p->use_tma_overlap = false;
     int dev = 0, sms = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const int want = env_int("SHARP_FRAME_CTAS_PER_SM", 0);
-    if (want > 0) bps = std::min(bps, want);
     if (bps < 1) return fail(p, SHARP_ECUDA, "frame kernel does not fit on an SM");
-    if (p->m >= 256) {   // whole clusters only; one scratch slot per cluster
-        const int cs = p->m == 256 ? kCluster256 : kCluster512;
-        const long long want_ctas = std::min<long long>({(long long)p->K * cs, (long long)sms * bps, (long long)p->slots_cap});
-        p->frame_grid = (int)std::max<long long>(cs, want_ctas / cs * cs);
-    } else {
-        p->frame_grid = std::min(p->frame_grid, sms * bps);
-    }
+    p->sms = sms;
+    p->device = dev;
+    p->frame_ctas_max = sms * bps;
+    update_frame_grid(p);
     CK(cudaMemcpyAsync(p->dp<int>(p->o_pos), p->pos.data(), p->pos.size() * 4, cudaMemcpyHostToDevice, p->stream));
     CK(cudaMemcpyAsync(p->dp<int>(p->o_tile_ptr), p->tile_ptr.data(), p->tile_ptr.size() * 4, cudaMemcpyHostToDevice, p->stream));
     if (!p->tile_frames.empty())
@@ -541,6 +484,15 @@ int sharp_set_frames(sharp_plan_t *p, const float *z_dev)
     p->cur = 0; p->vcur = 0;
     CK(cudaMemcpyAsync(p->dp<void>(p->o_c[0]), z_dev, p->npx() * 8, cudaMemcpyDeviceToDevice, p->stream));
     return adopt_frames(p);
+}
+
+int sharp_set_frame_slots(sharp_plan_t *p, int slots)
+{
+    if (!p) return SHARP_EINVAL;
+    if (slots < 0) return fail(p, SHARP_EINVAL, "slots must be >= 0");
+    p->slots_user = slots;
+    if (p->bound) update_frame_grid(p);
+    return SHARP_OK;
 }
 
 int sharp_set_probe_refine(sharp_plan_t *p, int every)

@@ -23,7 +23,7 @@ def _free_port():
 
 def _worker(rank, world, port, out):
     import bench
-    from paper_1602_01448_b200 import synth
+    import synth
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     args = argparse.Namespace(config=1, grid=4, iters=0)

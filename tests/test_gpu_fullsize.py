@@ -10,7 +10,7 @@ import pytest
 import torch
 
 import paper_1602_01448_b200 as sharp
-from paper_1602_01448_b200 import synth
+import synth
 
 pytestmark = pytest.mark.gpu
 

@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 import paper_1602_01448_b200 as sharp
-from paper_1602_01448_b200 import synth
+import synth
 
 pytestmark = pytest.mark.gpu
 
@@ -283,29 +283,6 @@ def test_edge_cases(oracle):
 def test_unbound_library_refuses(oracle):
     rec = sharp.Reconstruction(64, [[0, 0]], (64, 64), device=None)
     assert rec.lib.sharp_iterate(rec._plan, 1, 0.75) == sharp.SHARP_ESTATE
-    rec.close()
-
-
-def test_tma_overlap_path(oracle, monkeypatch):
-    """The bulk-tensor (TMA) variant of the overlap (SHARP_OVERLAP_TMA=1, read when the plan is made) on jittered
-    positions (odd box origins) and tile lists longer than its stage ring: operator parity and one RAAR step."""
-    monkeypatch.setenv("SHARP_OVERLAP_TMA", "1")
-    cfg = synth.reduced(synth.config(2), 5)
-    pos, shape, I, w0, obj, wt = synth.make(cfg)
-    rec = sharp.Reconstruction(cfg.m, pos, shape)
-    rec.set_intensities(I); rec.set_probe(wt)
-    f = _rc((cfg.K, cfg.m, cfg.m), 31)
-    got = rec.op_overlap(f).cpu().numpy()
-    want = oracle.L(f, wt, pos, shape)
-    den = oracle.overlap_den(wt, pos, shape)
-    assert rel(got * np.sqrt(den), want * np.sqrt(den)) < OP_TOL
-    assert np.all(got[den == 0] == 0)
-    a, A2, a_rms, thr = oracle.amplitudes(I)
-    z = (synth.exit_waves(cfg, obj, wt, pos) * (1 + 0.2 * _rc((cfg.K, cfg.m, cfg.m), 32))).astype(np.complex64)
-    rec.set_frames(z)
-    rec.iterate(2, cfg.beta)
-    want2 = oracle.raar(oracle.raar(z, wt, pos, shape, a, thr, cfg.beta), wt, pos, shape, a, thr, cfg.beta)
-    assert rel(rec.get_frames().cpu().numpy(), want2) < 3 * OP_TOL
     rec.close()
 
 

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import paper_1602_01448_b200 as sharp
-from paper_1602_01448_b200 import synth
+import synth
 
 
 @pytest.fixture(scope="module")

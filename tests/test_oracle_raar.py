@@ -7,7 +7,7 @@ import dataclasses
 import numpy as np
 import pytest
 
-from paper_1602_01448_b200 import synth
+import synth
 
 
 def _rc(shape, seed):

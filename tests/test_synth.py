@@ -2,7 +2,7 @@
 BASELINE.json's configs as read in SURVEY.md section 8(d)."""
 import numpy as np
 
-from paper_1602_01448_b200 import synth
+import synth
 
 
 def test_config_shapes_and_counts():
