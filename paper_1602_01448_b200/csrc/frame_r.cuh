@@ -29,6 +29,12 @@
 // per-thread base and a compile-time function of the register index (immediate offsets, no swizzle arithmetic);
 // the paddings (36, 144, 576 / 66, 132, 264, 528; row pitch 34) make every access bank-conflict free.
 // The amplitudes are stored in the order P3 reads them: a_int[(warp 32 + q) 32 + lane] (see slot_freq()).
+//
+// Latency: the state and the amplitudes of the next frame are pulled into L2 by one bulk prefetch each, a whole
+// frame ahead (measured: 262 us per launch at config 2 with it, 301 us without, and no better when issued later);
+// the position of the next frame is fetched a frame ahead as well.  Variants measured and dropped (config 2, us per
+// launch): amplitudes staged in shared memory by a bulk copy 298; object tile or amplitudes by cp.async into
+// slots of the exchange buffer the thread owns at that time 265 / 302; object tile requested before the state 297.
 #pragma once
 #include "fft_regs.cuh"
 #include "frame_common.cuh"
@@ -62,7 +68,7 @@ struct RCfg {
 };
 
 // Amplitude slot -> frequency: slot = (warp 32 + q) 32 + lane holds a(u, v), u = (warp SP + u1_low) + 32 u2,
-// v = lane + 32 v2, q = v2 + NLO u2 + NLO^2 u1_low.
+// v = lane + 32 v2, q = v2 + NLO u2 + NLO^2 u1_low: a warp's load of register q is 128 contiguous bytes.
 template <int M>
 SHARP_HD void slot_freq(int slot, int &u, int &v)
 {
@@ -226,7 +232,6 @@ __device__ __forceinline__ void r_tmem_ld16(unsigned taddr, float2 *x)
                  : "memory");
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
-
 template <int M, int MODE>
 __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(FrameArgs A)
 {
@@ -281,21 +286,29 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
 
     const float thr2 = A.sc->thr2;
     const float bm = A.bm, om = A.om;
-    float e_a = 0.f, e_q = 0.f, e_d = 0.f;     // per-frame fp32 partials
     double s_a = 0.0, s_q = 0.0, s_d = 0.0;
 
-    if (tid == 0 && (int)blockIdx.x < A.K) {
-        prefetch_l2_bulk(A.c_in + (size_t)blockIdx.x * M * M, M * M * 8);
-        if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)blockIdx.x * M * M, M * M * 4);
+    int xr_n = 0, xc_n = 0;      // position of the next frame, fetched one frame ahead
+    if ((int)blockIdx.x < A.K) {
+        xr_n = __ldg(A.pos + 2 * blockIdx.x);
+        xc_n = __ldg(A.pos + 2 * blockIdx.x + 1);
+        if (tid == 0) {
+            prefetch_l2_bulk(A.c_in + (size_t)blockIdx.x * M * M, M * M * 8);
+            if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)blockIdx.x * M * M, M * M * 4);
+        }
     }
 
     for (int i = blockIdx.x; i < A.K; i += gridDim.x) {
-        const int xr = A.pos[2 * i], xc = A.pos[2 * i + 1];
+        const int xr = xr_n, xc = xc_n;
         const size_t fbase = (size_t)i * M * M;
-        if (tid == 0 && i + (int)gridDim.x < A.K) {
-            const size_t nb = (size_t)(i + gridDim.x) * M * M;
-            prefetch_l2_bulk(A.c_in + nb, M * M * 8);
-            if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + nb, M * M * 4);
+        const bool more = i + (int)gridDim.x < A.K;
+        if (more) {
+            xr_n = __ldg(A.pos + 2 * (i + gridDim.x));
+            xc_n = __ldg(A.pos + 2 * (i + gridDim.x) + 1);
+            if (tid == 0) {
+                prefetch_l2_bulk(A.c_in + (size_t)(i + gridDim.x) * M * M, M * M * 8);
+                if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)(i + gridDim.x) * M * M, M * M * 4);
+            }
         }
         float2 v[32];
 
@@ -343,8 +356,8 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
                     const float2 dd = csub(v[k], zp);
                     sd += dd.x * dd.x + dd.y * dd.y;
                 }
-                e_q = sq;
-                e_d = sd;
+                s_q += (double)sq;
+                s_d += (double)sd;
             }
             dft<32, -1>(v);
             P::p1_store(tid, E, v);
@@ -389,10 +402,7 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
                         sa += dx * dx + dy * dy;
                     }
                 }
-                e_a = sa;
-                s_a += (double)e_a;
-                s_q += (double)e_q;
-                s_d += (double)e_d;
+                s_a += (double)sa;
                 __syncthreads();
                 continue;
             } else {
@@ -437,7 +447,6 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
             for (int k = 0; k < 32; ++k) st_stream(dst + (size_t)k * (NLO * M), v[k]);
         }
     }
-
     if (w_tmem) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();

@@ -639,6 +639,7 @@ int sharp_sync(sharp_plan_t *p)
 
 long long sharp_launch_count(const sharp_plan_t *p) { return p ? p->launches : 0; }
 
+
 int sharp_profile(sharp_plan_t *p, int on)
 {
     if (int rc = check_ready(p, false, false)) return rc;
