@@ -4,7 +4,11 @@ CTA or cluster per SM slot, many rounds, ragged last round).
 config 2 (2,500 frames 128x128): one teacher-forced RAAR iteration of the whole scan against the oracle, all frames.
 config 4 size (10,000 frames 256x256): the oracle cannot run the whole scan, so the frame-local operators are
 compared on sampled frames the oracle computes one by one (F, F*, P_a), plus Parseval over all frames; the overlap
-is compared on sampled object pixels by brute force over the frame list."""
+is compared on sampled object pixels by brute force over the frame list.
+config 4 and config 5 size with the factored state in use (test_fullsize_teacher_forced_step): one RAAR iteration
+from a generic state; on sampled frames the oracle's P_a and the RAAR formula evaluated in double from single
+frames and the object tiles under them; the two object arrays those tiles come from are themselves checked on
+sampled pixels by brute force over the frame list; the three metrics against plain torch reductions."""
 import numpy as np
 import pytest
 import torch
@@ -121,4 +125,86 @@ def test_config3_full_one_blind_iteration(oracle):
     want_psi = o.object()
     tol_p = max(5e-5, 10 * rel(o2.object()[lit], want_psi[lit]))
     assert rel(psi[lit], want_psi[lit]) < tol_p
+    rec.close()
+
+
+def _brute_force_pixels(psi, frames, w64, pos, m, shape, rng, n=24, tol=2e-5):
+    """Eq. 9 at sampled object pixels: sum over every frame covering the pixel, in double, from the frame list."""
+    checked = 0
+    for _ in range(n):
+        pr, pc = int(rng.integers(0, shape[0])), int(rng.integers(0, shape[1]))
+        rr, cc = pr - pos[:, 0], pc - pos[:, 1]
+        hit = np.nonzero((rr >= 0) & (rr < m) & (cc >= 0) & (cc < m))[0]
+        if hit.size == 0:
+            assert complex(psi[pr, pc]) == 0
+            continue
+        fv = torch.stack([frames[int(i), int(rr[i]), int(cc[i])] for i in hit]).cpu().numpy().astype(np.complex128)
+        wv = w64[rr[hit], cc[hit]]
+        den = np.sum(np.abs(wv) ** 2)
+        if den < 1e-3 * float(np.sum(np.abs(w64) ** 2)) / m ** 2 * hit.size:
+            continue                                # G5: ratio of rounding noise
+        want = np.sum(np.conj(wv) * fv) / den
+        assert abs(complex(psi[pr, pc]) - want) <= tol * max(abs(want), np.sqrt(np.sum(np.abs(fv) ** 2) / den) * 1e-1), (pr, pc)
+        checked += 1
+    assert checked >= n // 3
+
+
+@pytest.mark.parametrize("n", [4, 5])
+def test_fullsize_teacher_forced_step(oracle, n):
+    """configs 4 (10,000 frames 256x256) and 5 (1,600 frames 512x512) at full size, in the launch configuration
+    bench.py times (many rounds per cluster), with the factored state z = c + w T psi_v in use."""
+    cfg = synth.config(n)
+    pos = synth.positions(cfg)
+    K, m, shape, beta = cfg.K, cfg.m, cfg.shape, cfg.beta
+    rec = sharp.Reconstruction(m, pos, shape)
+    g = torch.Generator(device="cuda").manual_seed(1602 + n)
+    w = synth.true_probe(cfg)
+    # intensities of the right scale: |F(w x random-phase object)|^2-like level, random
+    I = torch.rand((K, m, m), device="cuda", generator=g) * float(2.0 * np.sum(np.abs(w) ** 2) / m ** 2)
+    rec.set_intensities(I)
+    rec.set_probe(w)
+    rec.set_object(None)
+    rec.iterate(2, beta)                               # generic state, psi_v != 0
+    z = rec.get_frames()
+    psi_z = rec.get_object()
+    y = rec.op_pa(z)
+    e0 = rec.errors()
+    rec.iterate(1, beta)
+    z1 = rec.get_frames()
+    psi_y = rec.get_object()
+    e1 = rec.errors()
+    w64 = w.astype(np.complex128)
+    A2 = float(I.double().sum()); thr = 1e-4 * np.sqrt(A2 / (K * m * m))
+    rng = np.random.default_rng(40 + n)
+    # the two object arrays, Eq. 9 by brute force on sampled pixels: psi_z = L z, psi_y = L y (= L z', identity O7)
+    _brute_force_pixels(psi_z, z, w64, pos, m, shape, rng)
+    _brute_force_pixels(psi_y, y, w64, pos, m, shape, rng)
+    _brute_force_pixels(psi_y, z1, w64, pos, m, shape, rng, tol=5e-5)
+    # sampled frames: P_a by the oracle, then step 5 (reading G1) typed out in double from the tiles
+    pz, py = psi_z.cpu().numpy().astype(np.complex128), psi_y.cpu().numpy().astype(np.complex128)
+    for i in [0, 1, K // 3, K // 2 + 1, K - 2, K - 1]:
+        zi = z[i].cpu().numpy()
+        ai = np.sqrt(np.maximum(I[i].cpu().numpy().astype(np.float64), 0))
+        yi = oracle.Pa(zi[None], ai[None], thr)[0]
+        assert rel(y[i].cpu().numpy(), yi) < 1e-5, i
+        r, c = int(pos[i, 0]), int(pos[i, 1])
+        want = 2 * beta * w64 * py[r:r + m, c:c + m] + (1 - 2 * beta) * yi + beta * (zi - w64 * pz[r:r + m, c:c + m])
+        assert rel(z1[i].cpu().numpy(), want) < 2e-5, (i, rel(z1[i].cpu().numpy(), want))
+    # the metrics at both states against plain torch reductions over all frames (double accumulation)
+    wt_ = torch.from_numpy(w).cuda()
+
+    def eps_q(zz, psi):
+        s = 0.0
+        for i in range(K):
+            r, c = int(pos[i, 0]), int(pos[i, 1])
+            s += float(torch.sum(torch.abs(wt_ * psi[r:r + m, c:c + m] - zz[i]).double() ** 2))
+        return np.sqrt(s / A2)
+
+    ea0 = float(torch.sqrt(torch.sum(torch.abs(y - z).double() ** 2) / A2))
+    assert abs(e0[0] / ea0 - 1) < 1e-4 and abs(e0[1] / eps_q(z, psi_z) - 1) < 1e-4, (e0, ea0)
+    y1 = rec.op_pa(z1)
+    ea1 = float(torch.sqrt(torch.sum(torch.abs(y1 - z1).double() ** 2) / A2))
+    ed1 = float(torch.sqrt(torch.sum(torch.abs(z1 - z).double() ** 2) / A2))
+    assert abs(e1[0] / ea1 - 1) < 1e-4 and abs(e1[2] / ed1 - 1) < 1e-4, (e1, ea1, ed1)
+    assert abs(e1[1] / eps_q(z1, psi_y) - 1) < 1e-4
     rec.close()

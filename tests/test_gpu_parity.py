@@ -2,8 +2,10 @@
 inputs.  Bars (BASELINE.json north_star): integer indexing bit-exact; each operator rel-L2 <= 1e-5; error metrics
 <= 1e-4 relative; free-running frames after 100 iterations <= 1e-3 where the iteration contracts.
 
-The scans are the BASELINE.json recipes on reduced rasters (sizes the oracle finishes in seconds) plus ragged
-random geometry; every size spans several FFT strips, several persistent-CTA rounds and a ragged tail."""
+The scans are the BASELINE.json recipes on reduced rasters (sizes the oracle finishes in seconds).  Every scan runs
+twice: with the default persistent grid (one CTA or cluster per frame at these sizes) and with the grid capped by
+`sharp_set_frame_slots` so that every CTA / cluster of the frame kernels loops over at least three frames with a
+ragged last round (the launch shape of the full-size configs: SLOTS below)."""
 import dataclasses
 
 import numpy as np
@@ -37,14 +39,22 @@ SCANS = {
 }
 
 
-@pytest.fixture(scope="module", params=list(SCANS))
+# frames in flight in "rounds" mode: K = 36 / 25 / 16 / 7 frames -> 8 / 9 / 6 / 4 rounds, the last one ragged
+SLOTS = {"m64": 5, "m128": 3, "m256": 3, "m512": 2}
+
+
+@pytest.fixture(scope="module", params=[(n, s) for n in SCANS for s in ("full", "rounds")], ids=lambda p: f"{p[0]}-{p[1]}")
 def scan(request):
-    n, grid = SCANS[request.param]
+    name, mode = request.param
+    n, grid = SCANS[name]
     cfg = synth.reduced(synth.config(n), grid)
     if cfg.kind == "fermat":
         cfg = dataclasses.replace(cfg, step=20)      # keep the 7 frames overlapping
     pos, shape, I, w0, obj, wt = synth.make(cfg)
     rec = sharp.Reconstruction(cfg.m, pos, shape)
+    if mode == "rounds":
+        rec.set_frame_slots(SLOTS[name])
+        assert cfg.K >= 3 * SLOTS[name] and cfg.K % SLOTS[name] != 0
     rec.set_intensities(I)
     rec.set_probe(wt)
     yield dict(cfg=cfg, pos=pos, shape=shape, I=I, w0=w0, obj=obj, wt=wt, rec=rec)
@@ -185,26 +195,131 @@ def test_probe_refinement_sequence_G10(scan, oracle):
     rec.set_probe(scan["wt"])
 
 
-def test_teacher_forced_trajectory_P9(scan, oracle):
-    """At several points of a free run, hand the GPU state to the oracle and advance both by one iteration."""
-    cfg, rec = scan["cfg"], scan["rec"]
-    a, A2, a_rms, thr = oracle.amplitudes(scan["I"])
-    rec.set_probe_refine(0)
-    rec.set_probe(scan["wt"])
-    rec.set_object(None)
+CHECKPOINTS = (1, 2, 5, 10, 20, 50, 100)
+TRAJ = {
+    # name: (config number, reduced grid or None for the full raster)
+    "cfg1-full": (1, None),       # 100 frames 64x64: the literal config 1
+    "cfg2-5x5": (2, 5),
+    "cfg3-5x5-blind": (3, 5),
+    "cfg5-7-blind": (5, 7),
+}
+
+
+def _traj_cfg(name):
+    n, grid = TRAJ[name]
+    cfg = synth.config(n)
+    if grid is not None:
+        cfg = synth.reduced(cfg, grid)
+    if cfg.kind == "fermat":
+        cfg = dataclasses.replace(cfg, step=20)
+    return cfg
+
+
+@pytest.mark.parametrize("name", list(TRAJ))
+def test_teacher_forced_checkpoints_P9(oracle, name):
+    """At iterations l in {1, 2, 5, 10, 20, 50, 100} of a free run the GPU state is handed to the oracle and both
+    advance by one iteration: frames <= 1e-5, metrics <= 1e-4 relative (decidable on the chaotic configs too).  On
+    the blind configs the probe is compared with a bar tied to the oracle's own sensitivity (Eq. 10 divides by
+    sum |psi|^2 of an unconstrained psi)."""
+    cfg = _traj_cfg(name)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    rec = sharp.Reconstruction(cfg.m, pos, shape)
+    if cfg.K > 8:
+        rec.set_frame_slots(max(2, cfg.K // 4 - 1))       # several rounds per CTA here as well
+    rec.set_intensities(I); rec.set_probe(w0); rec.set_object(None)
+    rec.set_probe_refine(cfg.refine_every)
+    a, A2, a_rms, thr = oracle.amplitudes(I)
+    rng = np.random.default_rng(9)
     done = 0
-    for upto in (1, 5, 12):
-        rec.iterate(upto - done, cfg.beta)
-        done = upto
+    for upto in CHECKPOINTS:
+        rec.iterate(upto - 1 - done, cfg.beta)
+        done = upto - 1
         z = rec.get_frames().cpu().numpy()
+        w = rec.get_probe().cpu().numpy()
         rec.iterate(1, cfg.beta)
         done += 1
         z1 = rec.get_frames().cpu().numpy()
-        want = oracle.raar(z, scan["wt"], scan["pos"], scan["shape"], a, thr, cfg.beta)
-        assert rel(z1, want) < OP_TOL, upto
+        o = oracle.Oracle(cfg.m, pos, shape, I, w, refine_every=cfg.refine_every)
+        o.set_frames(z)
+        o.it = done - 1
+        o.iterate(1, cfg.beta)
         e = rec.errors()
-        we = oracle.errors(want, z, scan["wt"], scan["pos"], scan["shape"], a, thr, A2)
-        assert np.allclose(e, we, rtol=EPS_TOL), (upto, e, we)
+        if not cfg.refine_every:
+            assert rel(z1, o.z) < OP_TOL, (name, upto, rel(z1, o.z))
+            assert np.allclose(e, o.errors(), rtol=EPS_TOL), (name, upto, e, o.errors())
+        else:
+            # blind starts (Gaussian probe x flat object) have a spectrum that crosses the G4 threshold smoothly, so
+            # a few |Z| ~ thr decisions per frame differ between fp32 and double: the bar is the oracle's own
+            # sensitivity to a 1e-7 perturbation of the same state (x10), floored at the operator tolerance
+            o2 = oracle.Oracle(cfg.m, pos, shape, I, w, refine_every=cfg.refine_every)
+            o2.set_frames((z * (1 + 1e-7 * rng.standard_normal(z.shape))).astype(np.complex64))
+            o2.it = done - 1
+            o2.iterate(1, cfg.beta)
+            tol_z = max(OP_TOL, 10 * rel(o2.z, o.z))
+            assert rel(z1, o.z) < tol_z, (name, upto, rel(z1, o.z), tol_z)
+            tol_w = max(2 * OP_TOL, 10 * rel(o2.w, o.w))
+            assert rel(rec.get_probe().cpu().numpy(), o.w) < tol_w, (name, upto, tol_w)
+            tol_e = max(EPS_TOL, 10 * float(np.abs(o2.errors() / o.errors() - 1).max()))
+            assert np.allclose(e, o.errors(), rtol=tol_e), (name, upto, e, o.errors(), tol_e)
+    rec.close()
+
+
+@pytest.mark.parametrize("name", list(TRAJ))
+def test_divergence_curve_P10(oracle, name):
+    """Free-running GPU trajectory against the free-running oracle on the chaotic configs (1, 2, 3, 5), beside the
+    oracle's own sensitivity to a 1e-7 relative perturbation of its inputs: the GPU curve must stay within 10x of
+    the self-sensitivity curve at every checkpoint.  The curves are printed."""
+    cfg = _traj_cfg(name)
+    pos, shape, I, w0, obj, wt = synth.make(cfg)
+    rec = sharp.Reconstruction(cfg.m, pos, shape)
+    rec.set_intensities(I); rec.set_probe(w0); rec.set_object(None)
+    rec.set_probe_refine(cfg.refine_every)
+    rng = np.random.default_rng(10)
+    Ip = (I.astype(np.float64) * (1 + 1e-7 * rng.standard_normal(I.shape))).astype(np.float32)
+    wp = (w0.astype(np.complex128) * (1 + 1e-7 * rng.standard_normal(w0.shape))).astype(np.complex64)
+    o = oracle.Oracle(cfg.m, pos, shape, I, w0, refine_every=cfg.refine_every)
+    o2 = oracle.Oracle(cfg.m, pos, shape, Ip, wp, refine_every=cfg.refine_every)
+    done = 0
+    rows = []
+    for upto in CHECKPOINTS:
+        rec.iterate(upto - done, cfg.beta); o.iterate(upto - done, cfg.beta); o2.iterate(upto - done, cfg.beta)
+        done = upto
+        d_gpu = rel(rec.get_frames().cpu().numpy(), o.z)
+        d_self = rel(o2.z, o.z)
+        rows.append((upto, d_gpu, d_self))
+    print(f"\n{name}: iteration, GPU-vs-oracle frames rel-L2, oracle self-sensitivity (1e-7 input perturbation)")
+    for r in rows:
+        print("   %4d  %.3e  %.3e" % r)
+    for upto, d_gpu, d_self in rows:
+        # 2 (saturation: decorrelated unit-norm trajectories) caps the bar; 3e-6 floors it at fp32 round-off level
+        assert d_gpu <= min(2.0, 10 * d_self + 3e-6), (name, upto, d_gpu, d_self)
+    rec.close()
+
+
+@pytest.mark.parametrize("beta", [0.55, 0.6])
+def test_low_beta_amplification(scan, oracle, beta):
+    """The factored state divides by 1 - 2 beta: fp32 error in psi_y is amplified by 1/(2 beta - 1),
+    10x at beta = 0.55.  Two RAAR steps (the second uses the factored form) against the oracle; bar = the operator
+    tolerance scaled by that factor (include/sharp_b200.h documents it)."""
+    cfg, rec = scan["cfg"], scan["rec"]
+    a, A2, a_rms, thr = oracle.amplitudes(scan["I"])
+    z = synth.exit_waves(cfg, scan["obj"], scan["wt"], scan["pos"]).astype(np.complex64)
+    z = (z * (1 + 0.2 * _rc(z.shape, 16))).astype(np.complex64)
+    rec.set_probe_refine(0)
+    rec.set_probe(scan["wt"])
+    rec.set_frames(z)
+    rec.iterate(1, beta)
+    want = oracle.raar(z, scan["wt"], scan["pos"], scan["shape"], a, thr, beta)
+    amp = 1.0 / (2 * beta - 1)
+    r1 = rel(rec.get_frames().cpu().numpy(), want)
+    rec.iterate(1, beta)
+    want2 = oracle.raar(want, scan["wt"], scan["pos"], scan["shape"], a, thr, beta)
+    r2 = rel(rec.get_frames().cpu().numpy(), want2)
+    print(f"\nbeta {beta}: step 1 rel {r1:.2e}, step 2 rel {r2:.2e} (amplification {amp:.0f}x)")
+    assert r1 < OP_TOL and r2 < OP_TOL * max(1.0, amp / 2), (r1, r2)
+    e = rec.errors()
+    we = oracle.errors(want2, want, scan["wt"], scan["pos"], scan["shape"], a, thr, A2)
+    assert np.allclose(e, we, rtol=EPS_TOL * max(1.0, amp / 2)), (e, we)
 
 
 def test_fixed_point_free_run_P10(scan, oracle):
@@ -216,8 +331,7 @@ def test_fixed_point_free_run_P10(scan, oracle):
     rec.set_intensities(I)
     rec.set_probe(scan["wt"])
     rec.set_frames(z0)
-    n = 100 if cfg.m <= 128 else 30
-    rec.iterate(n, cfg.beta)
+    rec.iterate(100, cfg.beta)
     z = rec.get_frames().cpu().numpy()
     assert rel(z, z0) < 1e-3
     assert rel(z, z0) < 2e-5          # in fact it stays at fp32 noise level
@@ -228,7 +342,10 @@ def test_fixed_point_free_run_P10(scan, oracle):
 
 def test_free_run_contracting_case_P10(oracle):
     """config-4 recipe (noise-free, beta 0.9, broad probe) on a 5x5 raster: the iteration contracts after a
-    transient, so GPU and oracle frames must agree after 100 free-running iterations."""
+    transient, so GPU and oracle frames must agree after 100 free-running iterations (<= 1e-3).
+    The three metrics are residuals at the 1e-4 level of ||a|| by then, i.e. small differences of nearly equal
+    frames, so their free-running bar is the oracle's own sensitivity (same run from inputs perturbed by 1e-7, x10),
+    floored at the 1e-4 of the north_star; teacher-forced (P9) the 1e-4 holds as it stands."""
     cfg = synth.reduced(synth.config(4), 5)
     pos, shape, I, w0, obj, wt = synth.make(cfg)
     rec = sharp.Reconstruction(cfg.m, pos, shape)
@@ -236,10 +353,18 @@ def test_free_run_contracting_case_P10(oracle):
     rec.iterate(100, cfg.beta)
     o = oracle.Oracle(cfg.m, pos, shape, I, w0)
     o.iterate(100, cfg.beta)
+    rng = np.random.default_rng(11)
+    Ip = (I.astype(np.float64) * (1 + 1e-7 * rng.standard_normal(I.shape))).astype(np.float32)
+    wp = (w0.astype(np.complex128) * (1 + 1e-7 * rng.standard_normal(w0.shape))).astype(np.complex64)
+    o2 = oracle.Oracle(cfg.m, pos, shape, Ip, wp)
+    o2.iterate(100, cfg.beta)
     z = rec.get_frames().cpu().numpy()
     assert rel(z, o.z) < 1e-3
-    e, eo = rec.errors(), o.errors()
-    assert np.allclose(e[:2], eo[:2], rtol=1e-2, atol=1e-7), (e, eo)
+    e, eo, eo2 = rec.errors(), o.errors(), o2.errors()
+    self_sens = np.abs(eo2 / eo - 1)
+    print(f"\ncontracting case, iteration 100: frames rel {rel(z, o.z):.2e} (oracle self-sensitivity {rel(o2.z, o.z):.2e}); "
+          f"metrics rel {np.abs(e / eo - 1)} (self-sensitivity {self_sens})")
+    assert np.all(np.abs(e / eo - 1) <= np.maximum(EPS_TOL, 10 * self_sens)), (e, eo, eo2)
     rec.close()
 
 
