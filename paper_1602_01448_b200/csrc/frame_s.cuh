@@ -1,0 +1,432 @@
+// frame_s.cuh -- the fused per-frame kernel for frames larger than one SM's shared memory (m = 256, 512): steps
+// a1-a4 and the frame-local half of a6 (same arithmetic as frame_r.cuh, see its header).
+//
+// A frame is processed in STRIPS of 8192 values (256 threads x 32 registers; 74 KB of shared memory, so two CTAs
+// with independent phases share an SM) by the CS CTAs of a thread-block cluster.  m = 32 NLO (NLO = 8, 16).
+//
+//   stage 1, column strips (WC = 8192/m columns each; CTA q takes strips q, q + CS, ...):
+//     P1  global -> registers, lanes along a row (coalesced 256 / 128 byte runs), registers i: rows r_lo + NLO i;
+//         z = c + w T psi_v formed on the fly; DFT32 over i -> u1.
+//     X1  CTA-wide exchange in shared memory (padded, bank-conflict free, immediate offsets).
+//     P2  registers (r_lo, sp): twiddle W_m^{u1 r_lo}, DFT_NLO over r_lo -> u2 (u = u1 + 32 u2); the result goes to
+//         the cluster's scratch frame in L2 in the order stage 2 reads it.
+//   -- cluster barrier --
+//   stage 2, row strips (WC rows each):
+//     P3  scratch -> registers (coalesced: thread = (c_lo, u_lo) x warp, registers j: columns c_lo + NLO j);
+//         DFT32 over j -> v1.
+//     X3  32 x 32 transposition inside the warp (pitch 34).
+//     P4  twiddle W_m^{v1 c_lo}, DFT_NLO over c_lo -> v2 (v = v1 + 32 v2); magnitude projection against the
+//         amplitudes (stored in exactly this order); the same steps backwards; scratch written in place.
+//   -- cluster barrier --
+//   stage 3, column strips: P2^-1 (scratch -> registers, same addresses the thread wrote in stage 1), X1^-1, P1^-1
+//     -> global.  Stage 1 of the cluster's next frame follows without a barrier (a thread only re-writes scratch
+//     locations it has just read itself).
+//
+// The scratch frame (m^2 c64 per cluster) is the only data that leaves the SM between F and F*; it is re-used for
+// every frame of the cluster and stays in L2 (evict-last policy; state / amplitudes stream with evict-first).
+// Scratch element (u, c): index ((u >> SPB) 32 + (c >> LB)) 32 + ((u & (SP-1)) << LB) + (c & (NLO-1)).
+#pragma once
+#include "fft_regs.cuh"
+#include "frame_common.cuh"
+
+namespace sharp {
+
+template <int M>
+struct SCfg {
+    static_assert(M == 256 || M == 512, "strip frame kernel: m = 256 or 512");
+    static constexpr int LB = (M == 256) ? 3 : 4, NLO = 1 << LB;
+    static constexpr int SPB = 5 - LB, SP = 1 << SPB;
+    static constexpr int NT = 256, NW = 8;
+    static constexpr int WC = 8192 / M, NSTR = M / WC;
+    static constexpr int RS = 1088, X2P = 34;
+    static constexpr int E_BYTES = NW * RS * 8, TW_BYTES = M * 8;
+    static constexpr int SMEM_BYTES = E_BYTES + TW_BYTES + 64;
+    // X1 offsets of register u1 (P1 side) and of register rho = r_lo + NLO sp (P2 side)
+    SHARP_HD static constexpr int x1u(int u1)
+    {
+        return M == 256 ? (u1 >> 2) * RS + 264 * (u1 & 3) : ((u1 >> 1) & 7) * RS + 256 * (u1 & 1) + 512 * (u1 >> 4);
+    }
+    SHARP_HD static constexpr int x1r(int rho)
+    {
+        return M == 256 ? 32 * (rho & 7) + 8 * (rho >> 3) : 16 * (rho & 15) + 512 * (rho >> 4);
+    }
+};
+
+// amplitude slot -> frequency (stage 2 order): slot = ((s2 8 + w3) 32 + q) 32 + lane, q = v2 + NLO u_lo
+template <int M>
+SHARP_HD void slot_freq_s(int slot, int &u, int &v)
+{
+    using C = SCfg<M>;
+    const int lane = slot & 31, q = (slot >> 5) & 31, uhi = slot >> 10;
+    u = (uhi << C::SPB) + (q >> C::LB);
+    v = lane + 32 * (q & (C::NLO - 1));
+}
+
+template <int M>
+struct SPass {
+    using C = SCfg<M>;
+    // ---- X1 -------------------------------------------------------------------------------------------------
+    SHARP_HD static int p1_base(int tid) { return (tid % C::WC) + C::WC * (tid / C::WC); }
+    SHARP_HD static void p1_store(int tid, float2 *E, const float2 *v)
+    {
+        float2 *b = E + p1_base(tid);
+#pragma unroll
+        for (int u1 = 0; u1 < 32; ++u1) b[C::x1u(u1)] = v[u1];
+    }
+    SHARP_HD static void p1_load(int tid, const float2 *E, float2 *v)
+    {
+        const float2 *b = E + p1_base(tid);
+#pragma unroll
+        for (int u1 = 0; u1 < 32; ++u1) v[u1] = b[C::x1u(u1)];
+    }
+    SHARP_HD static int p2_base(int tid)
+    {
+        const int w2 = tid >> 5, lane = tid & 31;
+        const int c_lo = lane & (C::NLO - 1), u1_lo = lane >> C::LB;
+        return w2 * C::RS + c_lo + (M == 256 ? 264 : 256) * u1_lo;
+    }
+    SHARP_HD static void p2_load(int tid, const float2 *E, float2 *v)
+    {
+        const float2 *b = E + p2_base(tid);
+#pragma unroll
+        for (int rho = 0; rho < 32; ++rho) v[rho] = b[C::x1r(rho)];
+    }
+    SHARP_HD static void p2_store(int tid, float2 *E, const float2 *v)
+    {
+        float2 *b = E + p2_base(tid);
+#pragma unroll
+        for (int rho = 0; rho < 32; ++rho) b[C::x1r(rho)] = v[rho];
+    }
+    // u1 of a P2 thread for spare index sp
+    SHARP_HD static int p2_u1(int tid, int sp)
+    {
+        const int w2 = tid >> 5, u1_lo = (tid & 31) >> C::LB;
+        return M == 256 ? 4 * w2 + u1_lo : 16 * sp + 2 * w2 + u1_lo;
+    }
+    // scratch index of register rho = u2 + NLO sp of a P2 thread working on column strip s1
+    SHARP_HD static int p2_scratch(int tid, int s1, int rho)
+    {
+        const int w2 = tid >> 5, lane = tid & 31;
+        const int u2 = rho & (C::NLO - 1), sp = rho >> C::LB;
+        const int uhi = M == 256 ? w2 + 8 * u2 : 8 * sp + w2 + 16 * u2;
+        const int j = M == 256 ? 4 * s1 + sp : s1;
+        return (uhi * 32 + j) * 32 + lane;
+    }
+    // twiddle + DFT_NLO over r_lo (forward) / inverse DFT_NLO + conjugate twiddle
+    template <bool INV>
+    SHARP_HD static void p2_math(int tid, const float2 *tw, float2 *v)
+    {
+#pragma unroll
+        for (int sp = 0; sp < C::SP; ++sp) {
+            float2 *p = v + C::NLO * sp;
+            const int u1 = p2_u1(tid, sp);
+            if (INV) Dft<C::NLO, +1, 1>::run(p);
+#pragma unroll
+            for (int rl = 1; rl < C::NLO; ++rl) {
+                const float2 t = tw[(u1 * rl) & (M - 1)];
+                p[rl] = INV ? cmulc(p[rl], t) : cmul(p[rl], t);
+            }
+            if (!INV) Dft<C::NLO, -1, 1>::run(p);
+        }
+    }
+    // ---- stage 2 ----------------------------------------------------------------------------------------------
+    SHARP_HD static int p3_scratch(int tid, int s2, int j) { return ((s2 * 8 + (tid >> 5)) * 32 + j) * 32 + (tid & 31); }
+    SHARP_HD static void x3_store_cols(int tid, float2 *E, const float2 *v)
+    {
+        float2 *b = E + (tid >> 5) * C::RS + (tid & 31);
+#pragma unroll
+        for (int v1 = 0; v1 < 32; ++v1) b[C::X2P * v1] = v[v1];
+    }
+    SHARP_HD static void x3_load_cols(int tid, const float2 *E, float2 *v)
+    {
+        const float2 *b = E + (tid >> 5) * C::RS + (tid & 31);
+#pragma unroll
+        for (int v1 = 0; v1 < 32; ++v1) v[v1] = b[C::X2P * v1];
+    }
+    SHARP_HD static void x3_load_rows(int tid, const float2 *E, float2 *v)
+    {
+        const float4 *b = reinterpret_cast<const float4 *>(E + (tid >> 5) * C::RS + C::X2P * (tid & 31));
+#pragma unroll
+        for (int q = 0; q < 32; q += 2) {
+            const float4 t = b[q >> 1];
+            v[q] = make_float2(t.x, t.y);
+            v[q + 1] = make_float2(t.z, t.w);
+        }
+    }
+    SHARP_HD static void x3_store_rows(int tid, float2 *E, const float2 *v)
+    {
+        float4 *b = reinterpret_cast<float4 *>(E + (tid >> 5) * C::RS + C::X2P * (tid & 31));
+#pragma unroll
+        for (int q = 0; q < 32; q += 2) b[q >> 1] = make_float4(v[q].x, v[q].y, v[q + 1].x, v[q + 1].y);
+    }
+    template <bool INV>
+    SHARP_HD static void p4_math(int tid, const float2 *tw, float2 *v)
+    {
+        const int v1 = tid & 31;
+        if (INV) {
+#pragma unroll
+            for (int ul = 0; ul < C::SP; ++ul) Dft<C::NLO, +1, 1>::run(v + C::NLO * ul);
+        }
+#pragma unroll
+        for (int cl = 1; cl < C::NLO; ++cl) {
+            const float2 t = tw[(v1 * cl) & (M - 1)];
+#pragma unroll
+            for (int ul = 0; ul < C::SP; ++ul) {
+                float2 &x = v[cl + C::NLO * ul];
+                x = INV ? cmulc(x, t) : cmul(x, t);
+            }
+        }
+        if (!INV) {
+#pragma unroll
+            for (int ul = 0; ul < C::SP; ++ul) Dft<C::NLO, -1, 1>::run(v + C::NLO * ul);
+        }
+    }
+};
+
+#if defined(__CUDACC__)
+
+__device__ __forceinline__ unsigned long long s_policy_evict_last()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ float2 s_ld_scratch(const float2 *p, unsigned long long pol)
+{
+    float2 v;
+    asm volatile("ld.global.cg.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ void s_st_scratch(float2 *p, float2 v, unsigned long long pol)
+{
+    asm volatile("st.global.cg.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y), "l"(pol) : "memory");
+}
+
+// Launched with cluster dimension CS; gridDim.x is a multiple of CS.  scratch: one m x m frame per cluster.
+template <int M, int MODE, int CS>
+__global__ void __launch_bounds__(SCfg<M>::NT, 2) k_frame_s(FrameArgs A)
+{
+    using C = SCfg<M>;
+    using P = SPass<M>;
+    constexpr int NLO = C::NLO, NT = C::NT, WC = C::WC;
+    static_assert(C::NSTR % CS == 0, "strips must divide evenly over the cluster");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *E = reinterpret_cast<float2 *>(smem_raw);
+    float2 *tw = reinterpret_cast<float2 *>(smem_raw + C::E_BYTES);
+
+    const int tid = threadIdx.x, wq = tid >> 5, lane = tid & 31;
+    const int col_l = tid % WC, r_lo = tid / WC;        // P1 identity
+    for (int k = tid; k < M; k += NT) {
+        float sn, cs;
+        sincospif(-2.0f * (float)k / (float)M, &sn, &cs);
+        tw[k] = make_float2(cs, sn);
+    }
+    __syncthreads();
+
+    const int crank = (int)cluster_rank();
+    const int cid = blockIdx.x / CS, nclusters = gridDim.x / CS;
+    float2 *scr = A.scratch + (size_t)cid * M * M;
+    const unsigned long long pol_keep = s_policy_evict_last();
+    const bool use_w = (MODE != FRAME_FFT) && A.psi_v != nullptr;
+    const float thr2 = A.sc->thr2;
+    const float bm = A.bm, om = A.om;
+    double s_a = 0.0, s_q = 0.0, s_d = 0.0;
+
+    // the cluster's next frame is pulled into L2 while this one is transformed, a CS-th per CTA
+    auto prefetch_frame = [&](int f) {
+        if (tid == 0 && f < A.K) {
+            const size_t fb = (size_t)f * M * M, part = (size_t)M * M / CS;
+            prefetch_l2_bulk(A.c_in + fb + crank * part, (unsigned)(part * 8));
+            if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + fb + crank * part, (unsigned)(part * 4));
+        }
+    };
+    prefetch_frame(cid);
+
+    for (int i = cid; i < A.K; i += nclusters) {
+        const int xr = __ldg(A.pos + 2 * i), xc = __ldg(A.pos + 2 * i + 1);
+        const size_t fbase = (size_t)i * M * M;
+        prefetch_frame(i + nclusters);
+        float2 v[32];
+
+        // ---------------- stage 1: column strips ------------------------------------------------------------
+        for (int s1 = crank; s1 < C::NSTR; s1 += CS) {
+            const int col = s1 * WC + col_l;
+            {
+                const float2 *cin = A.c_in + fbase + (size_t)r_lo * M + col;
+#pragma unroll
+                for (int k = 0; k < 32; ++k) v[k] = ld_stream(cin + (size_t)k * (NLO * M));
+                if (MODE == FRAME_FFT && A.conj_io) {
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) v[k].y = -v[k].y;
+                }
+                if (use_w) {
+                    const float2 *prow = A.psi_v + (size_t)(xr + r_lo) * A.nc + xc + col;
+                    const float2 *wrow = A.w_form + (size_t)r_lo * M + col;
+                    const size_t pstep = (size_t)NLO * A.nc;
+#pragma unroll
+                    for (int ch = 0; ch < 4; ++ch) {
+                        float2 pv[8], wv[8];
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) pv[k] = __ldg(prow + (size_t)(8 * ch + k) * pstep);
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) wv[k] = __ldg(wrow + (size_t)(8 * ch + k) * (NLO * M));
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) v[8 * ch + k] = cadd(v[8 * ch + k], cmul(wv[k], pv[k]));
+                    }
+                }
+                if constexpr (MODE == FRAME_ERR) {
+                    float sq = 0.f, sd = 0.f;
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) {
+                        const int r = r_lo + NLO * k;
+                        const size_t op = (size_t)(xr + r) * A.nc + xc + col;
+                        const float2 d = csub(cmul(__ldg(A.w_cur + r * M + col), __ldg(A.psi_z + op)), v[k]);
+                        sq += d.x * d.x + d.y * d.y;
+                        float2 zp = make_float2(0.f, 0.f);
+                        if (A.c_prev != nullptr) {
+                            zp = ld_stream(A.c_prev + fbase + (size_t)r * M + col);
+                            if (A.psi_v_prev != nullptr)
+                                zp = cadd(zp, cmul(__ldg(A.w_form_prev + r * M + col), __ldg(A.psi_v_prev + op)));
+                        }
+                        const float2 dd = csub(v[k], zp);
+                        sd += dd.x * dd.x + dd.y * dd.y;
+                    }
+                    s_q += (double)sq;
+                    s_d += (double)sd;
+                }
+                dft<32, -1>(v);
+            }
+            __syncthreads();                 // the previous strip's X1 readers are done
+            P::p1_store(tid, E, v);
+            __syncthreads();
+            P::p2_load(tid, E, v);
+            P::template p2_math<false>(tid, tw, v);
+#pragma unroll
+            for (int rho = 0; rho < 32; ++rho) s_st_scratch(scr + P::p2_scratch(tid, s1, rho), v[rho], pol_keep);
+        }
+        cluster_barrier();
+
+        // ---------------- stage 2: row strips ---------------------------------------------------------------
+        for (int s2 = crank; s2 < C::NSTR; s2 += CS) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = s_ld_scratch(scr + P::p3_scratch(tid, s2, j), pol_keep);
+            dft<32, -1>(v);
+            __syncwarp();
+            P::x3_store_cols(tid, E, v);
+            __syncwarp();
+            P::x3_load_rows(tid, E, v);
+            P::template p4_math<false>(tid, tw, v);
+            const int uhi = s2 * 8 + wq;
+            if constexpr (MODE == FRAME_FFT) {
+                const float inv_m = 1.0f / (float)M;
+#pragma unroll
+                for (int q = 0; q < 32; ++q) {
+                    int u, vv;
+                    slot_freq_s<M>((uhi * 32 + q) * 32 + lane, u, vv);
+                    float2 o = make_float2(v[q].x * inv_m, v[q].y * inv_m);
+                    if (A.conj_io) o.y = -o.y;
+                    A.c_out[fbase + (size_t)u * M + vv] = o;
+                }
+            } else {
+                const float *ap = A.a_int + fbase + (size_t)(uhi * 32) * 32 + lane;
+                if constexpr (MODE == FRAME_ERR) {
+                    const float fm = (float)M, inv_m = 1.0f / (float)M;
+                    float sa = 0.f;
+#pragma unroll
+                    for (int q = 0; q < 32; ++q) {
+                        const float a = __ldcs(ap + q * 32) * fm;
+                        const float mag2 = v[q].x * v[q].x + v[q].y * v[q].y;
+                        if (mag2 > thr2) {
+                            const float d = a - sqrtf(mag2) * inv_m;
+                            sa += d * d;
+                        } else {
+                            const float dx = a - v[q].x * inv_m, dy = v[q].y * inv_m;
+                            sa += dx * dx + dy * dy;
+                        }
+                    }
+                    s_a += (double)sa;
+                } else {
+#pragma unroll
+                    for (int q0 = 0; q0 < 32; q0 += 8) {
+                        float av[8];
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) av[k] = __ldcs(ap + (q0 + k) * 32);
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) {
+                            float2 &x = v[q0 + k];
+                            const float mag2 = x.x * x.x + x.y * x.y;
+                            const float oa = om * av[k];
+                            if (mag2 > thr2) {
+                                const float sc = fmaf(oa, rsqrtf(mag2), bm);
+                                x.x *= sc;
+                                x.y *= sc;
+                            } else {
+                                x.x = fmaf(bm, x.x, oa);
+                                x.y = bm * x.y;
+                            }
+                        }
+                    }
+                    P::template p4_math<true>(tid, tw, v);
+                    P::x3_store_rows(tid, E, v);
+                    __syncwarp();
+                    P::x3_load_cols(tid, E, v);
+                    dft<32, +1>(v);
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) s_st_scratch(scr + P::p3_scratch(tid, s2, j), v[j], pol_keep);
+                }
+            }
+            __syncwarp();
+        }
+        cluster_barrier();
+
+        // ---------------- stage 3: column strips ------------------------------------------------------------
+        if constexpr (MODE == FRAME_ITER) {
+            for (int s1 = crank; s1 < C::NSTR; s1 += CS) {
+#pragma unroll
+                for (int rho = 0; rho < 32; ++rho) v[rho] = s_ld_scratch(scr + P::p2_scratch(tid, s1, rho), pol_keep);
+                P::template p2_math<true>(tid, tw, v);
+                __syncthreads();             // the previous strip's X1 readers are done
+                P::p2_store(tid, E, v);
+                __syncthreads();
+                P::p1_load(tid, E, v);
+                dft<32, +1>(v);
+                float2 *dst = A.c_out + fbase + (size_t)r_lo * M + s1 * WC + col_l;
+#pragma unroll
+                for (int k = 0; k < 32; ++k) st_stream(dst + (size_t)k * (NLO * M), v[k]);
+            }
+        }
+    }
+
+    if constexpr (MODE == FRAME_ERR) {
+        // deterministic reduction: fixed xor-tree inside each warp, then the warp sums in warp order; one triple per CTA
+        __syncthreads();
+        double *red = reinterpret_cast<double *>(smem_raw);
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            s_a += __shfl_xor_sync(0xffffffffu, s_a, off);
+            s_q += __shfl_xor_sync(0xffffffffu, s_q, off);
+            s_d += __shfl_xor_sync(0xffffffffu, s_d, off);
+        }
+        if (lane == 0) {
+            red[3 * wq + 0] = s_a;
+            red[3 * wq + 1] = s_q;
+            red[3 * wq + 2] = s_d;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            double a = 0.0, q = 0.0, d = 0.0;
+            for (int w = 0; w < C::NW; ++w) {
+                a += red[3 * w + 0];
+                q += red[3 * w + 1];
+                d += red[3 * w + 2];
+            }
+            A.err_partials[3 * blockIdx.x + 0] = a;
+            A.err_partials[3 * blockIdx.x + 1] = q;
+            A.err_partials[3 * blockIdx.x + 2] = d;
+        }
+    }
+}
+
+#endif  // __CUDACC__
+
+}  // namespace sharp

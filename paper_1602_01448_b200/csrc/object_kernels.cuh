@@ -2,8 +2,9 @@
 // overlap with its object-space epilogues (a5 + the object half of a6), the illumination refinement (a7), the
 // amplitude preparation (a0) and small helpers.
 #pragma once
-#include "frame_kernel.cuh"
+#include "frame_common.cuh"
 #include "frame_r.cuh"
+#include "frame_s.cuh"
 
 namespace sharp {
 
@@ -69,22 +70,19 @@ __global__ void __launch_bounds__(256) k_frame_index(int m, int K, const int *po
 // ---------------------------------------------------------------------------------------------------------
 // a0 amplitudes:  a = sqrt(max(I, 0))  (reading G14), stored as a/m in the order in which the frame
 // kernel of this frame size meets the Fourier coefficients ("slots"): slot_freq() of frame_r.cuh for m <= 128,
-// the position space of frame_kernel.cuh (freq(x) = x / RB + RA (x % RB) on both axes) above.
+// slot_freq_s() of frame_s.cuh above.
 // Also per-block partial sums of max(I,0) in double (||a||^2, reading G12); k_scalars finishes them in a fixed
 // order.  k_amplitudes_natural is the inverse map (a_int -> a, for sharp_get_amplitudes).
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void amp_slot_freq(int m, int RA, int slot, int &u, int &v)
+__device__ __forceinline__ void amp_slot_freq(int m, int slot, int &u, int &v)
 {
     if (m == 64) slot_freq<64>(slot, u, v);
     else if (m == 128) slot_freq<128>(slot, u, v);
-    else {
-        const int RB = m / RA, q = slot / m, p = slot % m;
-        u = q / RB + RA * (q % RB);
-        v = p / RB + RA * (p % RB);
-    }
+    else if (m == 256) slot_freq_s<256>(slot, u, v);
+    else slot_freq_s<512>(slot, u, v);
 }
 
-__global__ void __launch_bounds__(256) k_amplitudes(int m, int RA, int K, const float *I, float *a_int,
+__global__ void __launch_bounds__(256) k_amplitudes(int m, int K, const float *I, float *a_int,
                                                      double *partials)
 {
     const size_t per_frame = (size_t)m * m;
@@ -94,7 +92,7 @@ __global__ void __launch_bounds__(256) k_amplitudes(int m, int RA, int K, const 
     for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
         const size_t i = g / per_frame;
         int u, v;
-        amp_slot_freq(m, RA, (int)(g - i * per_frame), u, v);
+        amp_slot_freq(m, (int)(g - i * per_frame), u, v);
         const float val = fmaxf(__ldg(I + i * per_frame + (size_t)u * m + v), 0.0f);
         acc += (double)val;
         a_int[g] = sqrtf(val) * inv_m;
@@ -109,14 +107,14 @@ __global__ void __launch_bounds__(256) k_amplitudes(int m, int RA, int K, const 
     if (threadIdx.x == 0) partials[blockIdx.x] = red[0];
 }
 
-__global__ void k_amplitudes_natural(int m, int RA, int K, const float *a_int, float *a)
+__global__ void k_amplitudes_natural(int m, int K, const float *a_int, float *a)
 {
     const size_t per_frame = (size_t)m * m;
     const size_t total = (size_t)K * per_frame;
     for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
         const size_t i = g / per_frame;
         int u, v;
-        amp_slot_freq(m, RA, (int)(g - i * per_frame), u, v);
+        amp_slot_freq(m, (int)(g - i * per_frame), u, v);
         a[i * per_frame + (size_t)u * m + v] = a_int[g] * (float)m;
     }
 }

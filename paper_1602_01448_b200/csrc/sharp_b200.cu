@@ -12,8 +12,8 @@
 #include <string>
 #include <vector>
 
-#include "frame_kernel.cuh"
 #include "frame_r.cuh"
+#include "frame_s.cuh"
 #include "object_kernels.cuh"
 
 using namespace sharp;
@@ -31,7 +31,6 @@ size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct sharp_plan_s {
     int m = 0, K = 0, nr = 0, nc = 0;
-    int E = 16;  // elements per thread of the frame kernel (radix of the strided FFT pass)
     int tiles_r = 0, tiles_c = 0;
     std::vector<int32_t> pos;          // K x 2
     std::vector<int32_t> tile_ptr;     // tiles + 1
@@ -134,28 +133,15 @@ int grid_for(size_t n, int per_block = 256, int cap = 160 * 16)
 }
 
 // ---- frame kernel dispatch -----------------------------------------------------------------------------------
-// m = 64, 128: the register-radix kernel of frame_r.cuh (whole frame on one SM).  m = 256, 512: strips in shared
-// memory, the row<->column transposition through a per-cluster scratch in L2 (frame_kernel.cuh).
-template <int M, int E, int NT, int MODE>
-int frame_smem_bytes()
-{
-    return FrameCfg<M, E, NT>::SMEM_BYTES + (E > 16 ? M * 8 : 0);
-}
+// m = 64, 128: the register-radix kernel of frame_r.cuh (whole frame on one SM).  m = 256, 512: strips of 8192
+// values per CTA, clusters of kCluster256 / kCluster512 CTAs per frame, row<->column transposition through one
+// scratch frame per cluster that lives in L2 (frame_s.cuh).
+constexpr int kCluster256 = 4, kCluster512 = 8;
+
+int cluster_size(int m) { return m <= 128 ? 1 : (m == 256 ? kCluster256 : kCluster512); }
 
 template <class KernelT>
-cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int *blocks_per_sm)
-{
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, kern, nt, smem);
-}
-
-// m >= 256: CS CTAs of a cluster share one frame, so that the scratch slots in flight (one per cluster) stay
-// inside L2: 148 x 512 KB at m = 256, 18 x 2 MB at m = 512.
-constexpr int kCluster256 = 2, kCluster512 = 8;
-
-template <class KernelT>
-cudaError_t launch_cluster(KernelT kern, int grid, int nt, int smem, int cs, cudaStream_t st, const FrameArgs &a)
+cudaLaunchConfig_t cluster_config(int grid, int nt, int smem, int cs, cudaStream_t st, cudaLaunchAttribute *attr)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof cfg);
@@ -163,13 +149,20 @@ cudaError_t launch_cluster(KernelT kern, int grid, int nt, int smem, int cs, cud
     cfg.blockDim = dim3(nt);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = cs;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    return cfg;
+}
+
+template <class KernelT>
+cudaError_t launch_cluster(KernelT kern, int grid, int nt, int smem, int cs, cudaStream_t st, const FrameArgs &a)
+{
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = cluster_config<KernelT>(grid, nt, smem, cs, st, attr);
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
@@ -181,12 +174,10 @@ int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
     case 64: k_frame_r<64, MODE><<<grid, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, p->stream>>>(a); break;
     case 128: k_frame_r<128, MODE><<<grid, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, p->stream>>>(a); break;
     case 256:
-        CK(launch_cluster(k_frame<256, 16, 256, MODE, kCluster256>, grid, 256, frame_smem_bytes<256, 16, 256, MODE>(),
-                          kCluster256, p->stream, a));
+        CK(launch_cluster(k_frame_s<256, MODE, kCluster256>, grid, SCfg<256>::NT, SCfg<256>::SMEM_BYTES, kCluster256, p->stream, a));
         break;
     case 512:
-        CK(launch_cluster(k_frame<512, 32, 256, MODE, kCluster512>, grid, 256, frame_smem_bytes<512, 32, 256, MODE>(),
-                          kCluster512, p->stream, a));
+        CK(launch_cluster(k_frame_s<512, MODE, kCluster512>, grid, SCfg<512>::NT, SCfg<512>::SMEM_BYTES, kCluster512, p->stream, a));
         break;
     default: return fail(p, SHARP_EINVAL, "unsupported frame size %d", p->m);
     }
@@ -194,14 +185,34 @@ int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
     return SHARP_OK;
 }
 
+// sets the shared-memory attribute and returns how many CTAs of the kernel can be resident on the device
+template <class KernelT>
+cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int cs, int sms, int *resident_ctas)
+{
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    if (cs == 1) {
+        int bps = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, nt, smem);
+        *resident_ctas = bps * sms;
+        return e;
+    }
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = cluster_config<KernelT>(sms * 8 / cs * cs, nt, smem, cs, nullptr, attr);
+    int nclusters = 0;
+    e = cudaOccupancyMaxActiveClusters(&nclusters, kern, &cfg);
+    *resident_ctas = nclusters * cs;
+    return e;
+}
+
 template <int MODE>
-cudaError_t frame_prepare_m(int m, int *bps)
+cudaError_t frame_prepare_m(int m, int sms, int *resident)
 {
     switch (m) {
-    case 64: return kernel_prepare(k_frame_r<64, MODE>, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, bps);
-    case 128: return kernel_prepare(k_frame_r<128, MODE>, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, bps);
-    case 256: return kernel_prepare(k_frame<256, 16, 256, MODE, kCluster256>, 256, frame_smem_bytes<256, 16, 256, MODE>(), bps);
-    default: return kernel_prepare(k_frame<512, 32, 256, MODE, kCluster512>, 256, frame_smem_bytes<512, 32, 256, MODE>(), bps);
+    case 64: return kernel_prepare(k_frame_r<64, MODE>, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, 1, sms, resident);
+    case 128: return kernel_prepare(k_frame_r<128, MODE>, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, 1, sms, resident);
+    case 256: return kernel_prepare(k_frame_s<256, MODE, kCluster256>, SCfg<256>::NT, SCfg<256>::SMEM_BYTES, kCluster256, sms, resident);
+    default: return kernel_prepare(k_frame_s<512, MODE, kCluster512>, SCfg<512>::NT, SCfg<512>::SMEM_BYTES, kCluster512, sms, resident);
     }
 }
 
@@ -265,7 +276,7 @@ int regather_psi_z(sharp_plan_t *p)
 // than there are frames; sharp_set_frame_slots lowers it (tests force several rounds per CTA that way)
 void update_frame_grid(sharp_plan_t *p)
 {
-    const int cs = p->m <= 128 ? 1 : (p->m == 256 ? kCluster256 : kCluster512);
+    const int cs = cluster_size(p->m);
     long long units = std::min<long long>(p->K, p->frame_ctas_max / cs);
     if (cs > 1) units = std::min<long long>(units, kMaxScratchCtas / cs);
     units = std::min<long long>(units, kMaxFrameSlots / cs);
@@ -324,7 +335,6 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     sharp_plan_t *p = new (std::nothrow) sharp_plan_s;
     if (!p) return fail(nullptr, SHARP_ENOMEM, "host allocation failed");
     p->m = m; p->K = K; p->nr = obj_rows; p->nc = obj_cols;
-    p->E = (m == 512) ? 32 : 16;
     p->pos.assign(pos_rc, pos_rc + 2 * (size_t)K);
     p->tiles_r = (obj_rows + TILE - 1) / TILE;
     p->tiles_c = (obj_cols + TILE - 1) / TILE;
@@ -367,7 +377,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->o_cross = take(p->nobj() * 8);
     for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
     // m <= 128 keeps the frame in shared memory; above, one L2 scratch slot per cluster of CTAs
-    const int cs_plan = m == 256 ? kCluster256 : kCluster512;
+    const int cs_plan = cluster_size(m);
     p->o_scratch = take(m <= 128 ? 256 : (size_t)std::min(K, kMaxScratchCtas / cs_plan) * m * m * 8);
     p->o_pos = take((size_t)K * 2 * 4);
     p->o_tile_ptr = take((ntiles + 1) * 4);
@@ -407,18 +417,19 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     p->ws_bytes = bytes;
     p->stream = static_cast<cudaStream_t>(cuda_stream);
     // size the persistent grid from the occupancy of the iteration kernel
-    int bps = 0;
-    CK(frame_prepare_m<FRAME_ITER>(p->m, &bps));
-    int bps2 = 0;
-    CK(frame_prepare_m<FRAME_FFT>(p->m, &bps2));
-    CK(frame_prepare_m<FRAME_ERR>(p->m, &bps2));
     int dev = 0, sms = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    if (bps < 1) return fail(p, SHARP_ECUDA, "frame kernel does not fit on an SM");
+    int resident = 0, resident2 = 0;
+    CK(frame_prepare_m<FRAME_ITER>(p->m, sms, &resident));
+    CK(frame_prepare_m<FRAME_FFT>(p->m, sms, &resident2));
+    resident = std::min(resident, resident2);
+    CK(frame_prepare_m<FRAME_ERR>(p->m, sms, &resident2));
+    resident = std::min(resident, resident2);
+    if (resident < 1) return fail(p, SHARP_ECUDA, "frame kernel does not fit on the device");
     p->sms = sms;
     p->device = dev;
-    p->frame_ctas_max = sms * bps;
+    p->frame_ctas_max = resident;
     update_frame_grid(p);
     CK(cudaMemcpyAsync(p->dp<int>(p->o_pos), p->pos.data(), p->pos.size() * 4, cudaMemcpyHostToDevice, p->stream));
     CK(cudaMemcpyAsync(p->dp<int>(p->o_tile_ptr), p->tile_ptr.data(), p->tile_ptr.size() * 4, cudaMemcpyHostToDevice, p->stream));
@@ -439,7 +450,7 @@ int sharp_set_intensities(sharp_plan_t *p, const float *I_dev)
 {
     if (int rc = check_ready(p, false, false)) return rc;
     if (!I_dev) return fail(p, SHARP_EINVAL, "I_dev is NULL");
-    k_amplitudes<<<p->amp_blocks, 256, 0, p->stream>>>(p->m, p->E, p->K, I_dev, p->dp<float>(p->o_a), p->dp<double>(p->o_partials));
+    k_amplitudes<<<p->amp_blocks, 256, 0, p->stream>>>(p->m, p->K, I_dev, p->dp<float>(p->o_a), p->dp<double>(p->o_partials));
     CK_LAUNCH("k_amplitudes");
     k_scalars<<<1, 32, 0, p->stream>>>(p->amp_blocks, p->dp<double>(p->o_partials), p->K, kTau, p->dp<DevScalars>(p->o_scalars));
     CK_LAUNCH("k_scalars");
@@ -596,7 +607,7 @@ int sharp_get_amplitudes(sharp_plan_t *p, float *out_dev)
 {
     if (int rc = check_ready(p, true, false)) return rc;
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
-    k_amplitudes_natural<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->E, p->K, p->dp<float>(p->o_a), out_dev);
+    k_amplitudes_natural<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<float>(p->o_a), out_dev);
     CK_LAUNCH("k_amplitudes_natural");
     return SHARP_OK;
 }
