@@ -22,6 +22,11 @@
 //     -> global.  Stage 1 of the cluster's next frame follows without a barrier (a thread only re-writes scratch
 //     locations it has just read itself).
 //
+// Measured at config-4 size (1,600 frames, us per launch): 256-thread CTAs in clusters of 4: 1098; 128-thread CTAs
+// (m = 256: strips of 16 columns, four CTAs per SM) in clusters of 8: 929, in clusters of 4: 1212; the probe parked in
+// tensor memory (4 x 128 columns per SM): 1821 (the allocations of the four resident CTAs serialise), dropped.
+// A bulk L2 prefetch of the cluster's next frame (what frame_r.cuh does) costs here: 926 with, 865 without (config 5:
+// 5.45 / 4.99 ms): the prefetched frames push the scratch frames out of L2.
 // The scratch frame (m^2 c64 per cluster) is the only data that leaves the SM between F and F*; it is re-used for
 // every frame of the cluster and stays in L2 (evict-last policy; state / amplitudes stream with evict-first).
 // Scratch element (u, c): index ((u >> SPB) 32 + (c >> LB)) 32 + ((u & (SP-1)) << LB) + (c & (NLO-1)).
@@ -31,40 +36,48 @@
 
 namespace sharp {
 
-template <int M>
+template <int M, int NT_>
 struct SCfg {
-    static_assert(M == 256 || M == 512, "strip frame kernel: m = 256 or 512");
+    static_assert((M == 256 && (NT_ == 256 || NT_ == 128)) || (M == 512 && NT_ == 256), "strip frame kernel: m = 256 or 512");
     static constexpr int LB = (M == 256) ? 3 : 4, NLO = 1 << LB;
     static constexpr int SPB = 5 - LB, SP = 1 << SPB;
-    static constexpr int NT = 256, NW = 8;
-    static constexpr int WC = 8192 / M, NSTR = M / WC;
+    static constexpr int NT = NT_, NW = NT / 32;
+    static constexpr int WC = NT * 32 / M, NSTR = M / WC;     // strip width (columns / rows), strips per stage
+    static constexpr int UW = WC >> SPB;                      // P3 warps (blocks of SP rows) per row strip == NW
     static constexpr int RS = 1088, X2P = 34;
     static constexpr int E_BYTES = NW * RS * 8, TW_BYTES = M * 8;
     static constexpr int SMEM_BYTES = E_BYTES + TW_BYTES + 64;
-    // X1 offsets of register u1 (P1 side) and of register rho = r_lo + NLO sp (P2 side)
+    static constexpr bool HALF = (NT == 128);                 // m = 256 in strips of 16 columns
+    static_assert(UW == NW, "row strips: one P3 warp per SP rows");
+    // X1 offsets of register u1 (P1 side) and of register rho = r_lo + NLO sp (P2 side); region = P2 warp
     SHARP_HD static constexpr int x1u(int u1)
     {
-        return M == 256 ? (u1 >> 2) * RS + 264 * (u1 & 3) : ((u1 >> 1) & 7) * RS + 256 * (u1 & 1) + 512 * (u1 >> 4);
+        return HALF ? ((u1 >> 2) & 3) * RS + 136 * (u1 & 3) + 544 * (u1 >> 4)
+             : M == 256 ? (u1 >> 2) * RS + 264 * (u1 & 3)
+                        : ((u1 >> 1) & 7) * RS + 256 * (u1 & 1) + 512 * (u1 >> 4);
     }
     SHARP_HD static constexpr int x1r(int rho)
     {
-        return M == 256 ? 32 * (rho & 7) + 8 * (rho >> 3) : 16 * (rho & 15) + 512 * (rho >> 4);
+        return HALF ? 16 * (rho & 7) + 8 * ((rho >> 3) & 1) + 544 * (rho >> 4)
+             : M == 256 ? 32 * (rho & 7) + 8 * (rho >> 3)
+                        : 16 * (rho & 15) + 512 * (rho >> 4);
     }
+    SHARP_HD static constexpr int x1lane(int u1_lo) { return (HALF ? 136 : M == 256 ? 264 : 256) * u1_lo; }
 };
 
 // amplitude slot -> frequency (stage 2 order): slot = ((s2 8 + w3) 32 + q) 32 + lane, q = v2 + NLO u_lo
 template <int M>
 SHARP_HD void slot_freq_s(int slot, int &u, int &v)
 {
-    using C = SCfg<M>;
+    using C = SCfg<M, 256>;
     const int lane = slot & 31, q = (slot >> 5) & 31, uhi = slot >> 10;
     u = (uhi << C::SPB) + (q >> C::LB);
     v = lane + 32 * (q & (C::NLO - 1));
 }
 
-template <int M>
+template <int M, int NT_>
 struct SPass {
-    using C = SCfg<M>;
+    using C = SCfg<M, NT_>;
     // ---- X1 -------------------------------------------------------------------------------------------------
     SHARP_HD static int p1_base(int tid) { return (tid % C::WC) + C::WC * (tid / C::WC); }
     SHARP_HD static void p1_store(int tid, float2 *E, const float2 *v)
@@ -83,7 +96,7 @@ struct SPass {
     {
         const int w2 = tid >> 5, lane = tid & 31;
         const int c_lo = lane & (C::NLO - 1), u1_lo = lane >> C::LB;
-        return w2 * C::RS + c_lo + (M == 256 ? 264 : 256) * u1_lo;
+        return w2 * C::RS + c_lo + C::x1lane(u1_lo);
     }
     SHARP_HD static void p2_load(int tid, const float2 *E, float2 *v)
     {
@@ -101,15 +114,15 @@ struct SPass {
     SHARP_HD static int p2_u1(int tid, int sp)
     {
         const int w2 = tid >> 5, u1_lo = (tid & 31) >> C::LB;
-        return M == 256 ? 4 * w2 + u1_lo : 16 * sp + 2 * w2 + u1_lo;
+        return C::HALF ? 16 * (sp >> 1) + 4 * w2 + u1_lo : M == 256 ? 4 * w2 + u1_lo : 16 * sp + 2 * w2 + u1_lo;
     }
     // scratch index of register rho = u2 + NLO sp of a P2 thread working on column strip s1
     SHARP_HD static int p2_scratch(int tid, int s1, int rho)
     {
         const int w2 = tid >> 5, lane = tid & 31;
         const int u2 = rho & (C::NLO - 1), sp = rho >> C::LB;
-        const int uhi = M == 256 ? w2 + 8 * u2 : 8 * sp + w2 + 16 * u2;
-        const int j = M == 256 ? 4 * s1 + sp : s1;
+        const int uhi = C::HALF ? 4 * (sp >> 1) + w2 + 8 * u2 : M == 256 ? w2 + 8 * u2 : 8 * sp + w2 + 16 * u2;
+        const int j = C::HALF ? 2 * s1 + (sp & 1) : M == 256 ? 4 * s1 + sp : s1;
         return (uhi * 32 + j) * 32 + lane;
     }
     // twiddle + DFT_NLO over r_lo (forward) / inverse DFT_NLO + conjugate twiddle
@@ -130,7 +143,7 @@ struct SPass {
         }
     }
     // ---- stage 2 ----------------------------------------------------------------------------------------------
-    SHARP_HD static int p3_scratch(int tid, int s2, int j) { return ((s2 * 8 + (tid >> 5)) * 32 + j) * 32 + (tid & 31); }
+    SHARP_HD static int p3_scratch(int tid, int s2, int j) { return ((s2 * C::NW + (tid >> 5)) * 32 + j) * 32 + (tid & 31); }
     SHARP_HD static void x3_store_cols(int tid, float2 *E, const float2 *v)
     {
         float2 *b = E + (tid >> 5) * C::RS + (tid & 31);
@@ -203,11 +216,11 @@ __device__ __forceinline__ void s_st_scratch(float2 *p, float2 v, unsigned long 
 }
 
 // Launched with cluster dimension CS; gridDim.x is a multiple of CS.  scratch: one m x m frame per cluster.
-template <int M, int MODE, int CS>
-__global__ void __launch_bounds__(SCfg<M>::NT, 2) k_frame_s(FrameArgs A)
+template <int M, int NT_, int MODE, int CS>
+__global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
 {
-    using C = SCfg<M>;
-    using P = SPass<M>;
+    using C = SCfg<M, NT_>;
+    using P = SPass<M, NT_>;
     constexpr int NLO = C::NLO, NT = C::NT, WC = C::WC;
     static_assert(C::NSTR % CS == 0, "strips must divide evenly over the cluster");
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -232,20 +245,9 @@ __global__ void __launch_bounds__(SCfg<M>::NT, 2) k_frame_s(FrameArgs A)
     const float bm = A.bm, om = A.om;
     double s_a = 0.0, s_q = 0.0, s_d = 0.0;
 
-    // the cluster's next frame is pulled into L2 while this one is transformed, a CS-th per CTA
-    auto prefetch_frame = [&](int f) {
-        if (tid == 0 && f < A.K) {
-            const size_t fb = (size_t)f * M * M, part = (size_t)M * M / CS;
-            prefetch_l2_bulk(A.c_in + fb + crank * part, (unsigned)(part * 8));
-            if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + fb + crank * part, (unsigned)(part * 4));
-        }
-    };
-    prefetch_frame(cid);
-
     for (int i = cid; i < A.K; i += nclusters) {
         const int xr = __ldg(A.pos + 2 * i), xc = __ldg(A.pos + 2 * i + 1);
         const size_t fbase = (size_t)i * M * M;
-        prefetch_frame(i + nclusters);
         float2 v[32];
 
         // ---------------- stage 1: column strips ------------------------------------------------------------
@@ -304,19 +306,32 @@ __global__ void __launch_bounds__(SCfg<M>::NT, 2) k_frame_s(FrameArgs A)
 #pragma unroll
             for (int rho = 0; rho < 32; ++rho) s_st_scratch(scr + P::p2_scratch(tid, s1, rho), v[rho], pol_keep);
         }
-        cluster_barrier();
+        // this thread's 32 amplitudes of a row strip are requested well ahead of the projection: for the first strip
+        // between the arrive and the wait of the cluster barrier, for the others before the forward transform
+        float av_all[32];
+        auto load_amplitudes = [&](int s2) {
+            if (MODE == FRAME_ITER) {
+                const float *ap0 = A.a_int + fbase + (size_t)((s2 * C::NW + wq) * 32) * 32 + lane;
+#pragma unroll
+                for (int q = 0; q < 32; ++q) av_all[q] = __ldcs(ap0 + q * 32);
+            }
+        };
+        cluster_arrive();
+        load_amplitudes(crank);
+        cluster_wait();
 
         // ---------------- stage 2: row strips ---------------------------------------------------------------
         for (int s2 = crank; s2 < C::NSTR; s2 += CS) {
 #pragma unroll
             for (int j = 0; j < 32; ++j) v[j] = s_ld_scratch(scr + P::p3_scratch(tid, s2, j), pol_keep);
+            if (s2 != crank) load_amplitudes(s2);
             dft<32, -1>(v);
             __syncwarp();
             P::x3_store_cols(tid, E, v);
             __syncwarp();
             P::x3_load_rows(tid, E, v);
             P::template p4_math<false>(tid, tw, v);
-            const int uhi = s2 * 8 + wq;
+            const int uhi = s2 * C::NW + wq;
             if constexpr (MODE == FRAME_FFT) {
                 const float inv_m = 1.0f / (float)M;
 #pragma unroll
@@ -350,7 +365,7 @@ __global__ void __launch_bounds__(SCfg<M>::NT, 2) k_frame_s(FrameArgs A)
                     for (int q0 = 0; q0 < 32; q0 += 8) {
                         float av[8];
 #pragma unroll
-                        for (int k = 0; k < 8; ++k) av[k] = __ldcs(ap + (q0 + k) * 32);
+                        for (int k = 0; k < 8; ++k) av[k] = av_all[q0 + k];
 #pragma unroll
                         for (int k = 0; k < 8; ++k) {
                             float2 &x = v[q0 + k];

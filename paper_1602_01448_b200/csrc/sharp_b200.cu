@@ -22,7 +22,6 @@ namespace {
 
 constexpr double kTau = 1e-4;  // reading G4: thr = tau * a_rms
 constexpr int kMaxFrameSlots = 1024;   // upper bound on the persistent frame grid (sizes the error partials)
-constexpr int kMaxScratchCtas = 2 * 160;  // m >= 256: CTAs whose clusters own an L2 scratch slot
 thread_local std::string g_plan_error = "";
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
@@ -136,7 +135,17 @@ int grid_for(size_t n, int per_block = 256, int cap = 160 * 16)
 // m = 64, 128: the register-radix kernel of frame_r.cuh (whole frame on one SM).  m = 256, 512: strips of 8192
 // values per CTA, clusters of kCluster256 / kCluster512 CTAs per frame, row<->column transposition through one
 // scratch frame per cluster that lives in L2 (frame_s.cuh).
-constexpr int kCluster256 = 4, kCluster512 = 8;
+#ifndef SHARP_NT256
+#define SHARP_NT256 128
+#endif
+#ifndef SHARP_CS256
+#define SHARP_CS256 8
+#endif
+constexpr int kNT256 = SHARP_NT256;      // threads per CTA (strip of 32 kNT256 values) at m = 256
+constexpr int kCluster256 = SHARP_CS256, kCluster512 = 8;
+
+// m >= 256: clusters in flight, each owning one scratch frame (m^2 c64) that should stay resident in L2
+int max_scratch_clusters(int m) { return m == 256 ? 80 : 40; }
 
 int cluster_size(int m) { return m <= 128 ? 1 : (m == 256 ? kCluster256 : kCluster512); }
 
@@ -174,10 +183,10 @@ int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
     case 64: k_frame_r<64, MODE><<<grid, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, p->stream>>>(a); break;
     case 128: k_frame_r<128, MODE><<<grid, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, p->stream>>>(a); break;
     case 256:
-        CK(launch_cluster(k_frame_s<256, MODE, kCluster256>, grid, SCfg<256>::NT, SCfg<256>::SMEM_BYTES, kCluster256, p->stream, a));
+        CK(launch_cluster(k_frame_s<256, kNT256, MODE, kCluster256>, grid, kNT256, SCfg<256, kNT256>::SMEM_BYTES, kCluster256, p->stream, a));
         break;
     case 512:
-        CK(launch_cluster(k_frame_s<512, MODE, kCluster512>, grid, SCfg<512>::NT, SCfg<512>::SMEM_BYTES, kCluster512, p->stream, a));
+        CK(launch_cluster(k_frame_s<512, 256, MODE, kCluster512>, grid, 256, SCfg<512, 256>::SMEM_BYTES, kCluster512, p->stream, a));
         break;
     default: return fail(p, SHARP_EINVAL, "unsupported frame size %d", p->m);
     }
@@ -211,8 +220,8 @@ cudaError_t frame_prepare_m(int m, int sms, int *resident)
     switch (m) {
     case 64: return kernel_prepare(k_frame_r<64, MODE>, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, 1, sms, resident);
     case 128: return kernel_prepare(k_frame_r<128, MODE>, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, 1, sms, resident);
-    case 256: return kernel_prepare(k_frame_s<256, MODE, kCluster256>, SCfg<256>::NT, SCfg<256>::SMEM_BYTES, kCluster256, sms, resident);
-    default: return kernel_prepare(k_frame_s<512, MODE, kCluster512>, SCfg<512>::NT, SCfg<512>::SMEM_BYTES, kCluster512, sms, resident);
+    case 256: return kernel_prepare(k_frame_s<256, kNT256, MODE, kCluster256>, kNT256, SCfg<256, kNT256>::SMEM_BYTES, kCluster256, sms, resident);
+    default: return kernel_prepare(k_frame_s<512, 256, MODE, kCluster512>, 256, SCfg<512, 256>::SMEM_BYTES, kCluster512, sms, resident);
     }
 }
 
@@ -278,7 +287,7 @@ void update_frame_grid(sharp_plan_t *p)
 {
     const int cs = cluster_size(p->m);
     long long units = std::min<long long>(p->K, p->frame_ctas_max / cs);
-    if (cs > 1) units = std::min<long long>(units, kMaxScratchCtas / cs);
+    if (cs > 1) units = std::min<long long>(units, max_scratch_clusters(p->m));
     units = std::min<long long>(units, kMaxFrameSlots / cs);
     if (p->slots_user > 0) units = std::min<long long>(units, p->slots_user);
     p->frame_grid = (int)std::max<long long>(1, units) * cs;
@@ -378,7 +387,7 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     for (int j = 0; j < 4; ++j) p->o_w[j] = take((size_t)m * m * 8);
     // m <= 128 keeps the frame in shared memory; above, one L2 scratch slot per cluster of CTAs
     const int cs_plan = cluster_size(m);
-    p->o_scratch = take(m <= 128 ? 256 : (size_t)std::min(K, kMaxScratchCtas / cs_plan) * m * m * 8);
+    p->o_scratch = take(m <= 128 ? 256 : (size_t)std::min(K, max_scratch_clusters(m)) * m * m * 8);
     p->o_pos = take((size_t)K * 2 * 4);
     p->o_tile_ptr = take((ntiles + 1) * 4);
     p->o_tile_frames = take(std::max<size_t>(p->tile_frames.size(), 1) * 4);
