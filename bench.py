@@ -17,7 +17,10 @@ metric is frame-iterations/s = ranks * K_frames * iters * steps / time.
   cpu_baseline / --impl reference   the CPU oracle (oracle/, double precision, OpenMP over the host cores) as it
              stands, on a bounded sub-raster sample of the same recipe
 
-N > 1 (torchrun): every rank reconstructs its own scan (same recipe, seed + rank), no data-path collective:
+  secondary  the default run (config 2, m = 128) also measures config 4 (m = 256, full size) the same way and
+             reports it under `secondary` (BASELINE.json's metric names both sizes); --no-secondary skips it
+
+N > 1 (torchrun): every rank reconstructs its own scan (same recipe, seed + 1000 rank), no data-path collective:
 weak scaling.  Timing is the max over ranks.
 """
 from __future__ import annotations
@@ -53,6 +56,7 @@ def parse():
     ap.add_argument("--grid", type=int, default=0, help="reduce the raster to grid x grid (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the config-4 (m = 256) block of the default run")
     return ap.parse_args()
 
 
@@ -202,26 +206,26 @@ def job_value(world, K, iters, steps, ms):
 
 
 # ---- our arm ----------------------------------------------------------------------------------------------------
-def run_ours(args):
+def spans_per_step(cfg, iters):
+    """kernel launches the library brackets with events in one step (sharp_profile caps the record at 8192)."""
+    per_it = 2 + (4 if cfg.refine_every else 0)
+    return per_it * iters + 8
+
+
+def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e, sample_clocks):
+    """One workload (BASELINE.json configs[config_number-1]) on this rank: device-resident throughput, per-kernel
+    durations and the roofline of the fused frame kernel, and the host-buffer end-to-end number."""
+    import dataclasses
     import torch
     import paper_1602_01448_b200 as sharp
     import synth
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the library has no CPU path (use --impl reference for the oracle)")
-    sharp.load_library()
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
-
-    cfg, iters = workload(args, rank)
+    cfg = synth.config(config_number)
+    if args.grid:
+        cfg = synth.reduced(cfg, args.grid)
+    if rank:
+        cfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    iters = args.iters or cfg.iters
     pos, shape, I, w0, obj, wt = synth.make(cfg)
     K, m = cfg.K, cfg.m
     I_host = torch.from_numpy(np.ascontiguousarray(I)).pin_memory()
@@ -246,16 +250,16 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         eps = step()
 
     # ---- timed region: device-resident ------------------------------------------------------------------------
-    sampler = ClockSampler(local) if rank == 0 else None
+    sampler = ClockSampler(dev.index) if sample_clocks else None
     barrier()
     l0 = rec.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         eps = step()
     e1.record()
     barrier()
@@ -263,11 +267,11 @@ def run_ours(args):
     launches = rec.launch_count() - l0
     clocks = sampler.stop() if sampler else None
     ms = max_over_ranks(ms, dist, dev)
-    value = job_value(world, K, iters, args.steps, ms)
+    value = job_value(world, K, iters, steps, ms)
 
     # ---- second pass over the same steps with events around every launch: per-kernel durations -----------------
     rec.profile(True)
-    nprof = max(1, min(args.steps, 8192 // max(1, 2 * iters + 8)))
+    nprof = max(1, min(steps, 8192 // spans_per_step(cfg, iters)))
     for _ in range(nprof):
         step()
     prof = rec.profile_read()
@@ -278,26 +282,32 @@ def run_ours(args):
     achieved = alg_bytes / (f_ms / f_n * 1e-3) / 1e9 if f_n else None
     tot_ms = sum(v[0] for v in prof.values())
     roofline = {
-        "kernel": "k_frame<FRAME_ITER> (fused split-add / FFT2 / magnitude projection / IFFT2 / frame combine)",
+        "kernel": ("k_frame_r" if m <= 128 else "k_frame_s") + "<FRAME_ITER> (fused split-add / FFT2 / magnitude "
+                  "projection / IFFT2 / frame combine)",
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
         "frac": (achieved / peak) if achieved else None, "traffic": None,
+        "frac_of_nominal_8TBs": (achieved / 8000.0) if achieved else None,
         "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
         "avg_launch_ms": f_ms / f_n if f_n else None, "launches_timed": f_n,
         "share_of_kernel_time": {k: (v[0] / tot_ms if tot_ms else None) for k, v in prof.items()},
         "avg_ms": {k: (v[0] / v[1] if v[1] else None) for k, v in prof.items()},
     }
-    traffic_file = os.path.join(ROOT, "profiles", f"traffic_cfg{args.config}.json")
-    if os.path.exists(traffic_file):         # dram bytes per launch read off a committed ncu --set full capture
+    traffic_file = os.path.join(ROOT, "profiles", f"traffic_cfg{config_number}.json")
+    if os.path.exists(traffic_file) and not args.grid:
+        # DRAM bytes per launch of the frame kernel, read off this round's committed `ncu --set full` capture of the
+        # same kernel at this config (profiles/r02_summary.md names the command); null when there is no capture
         try:
             with open(traffic_file) as f:
-                roofline["traffic"] = json.load(f).get("frame_kernel_dram_bytes_per_launch")
+                t = json.load(f)
+            roofline["traffic"] = t.get("frame_kernel_dram_bytes_per_launch")
+            roofline["traffic_source"] = t.get("source")
         except Exception:
             pass
 
     # ---- end to end: host buffers in, host buffers out ---------------------------------------------------------
     e2e = None
-    if not args.no_e2e:
-        n_e2e = max(1, min(args.steps, 5))
+    if want_e2e:
+        n_e2e = max(1, min(steps, 5))
         rec.reconstruct_host(I_host, w_host, iters, cfg.beta)      # warm-up (allocates the pinned outputs)
         barrier()
         t0 = time.perf_counter()
@@ -311,6 +321,49 @@ def run_ours(args):
                "d2h_bytes_per_step": int(shape[0] * shape[1] * 8 + m * m * 8 + 12),
                "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
                "api": "sharp_reconstruct_host (pinned host intensities + probe in; object, probe, residuals out)"}
+    eps0 = None
+    if hasattr(rec, "eps0"):
+        try:
+            eps0 = float(rec.eps0(obj))      # Eq. 14: error against the known synthetic object (the last step's result)
+        except Exception:
+            eps0 = None
+    rec.close()
+    del rec, I_dev
+    torch.cuda.empty_cache()
+    return {
+        "value": value, "ms": ms, "steps": steps, "iters": iters, "eps": [float(x) for x in eps], "eps0": eps0,
+        "launches": int(launches), "clocks": clocks, "roofline": roofline, "e2e": e2e,
+        "workload": workload_name(cfg, iters), "K": K, "m": m,
+        "l2": "inputs larger than L2 (frame state 2x%.0f MB + amplitudes %.0f MB per iteration vs 126 MB L2)"
+              % (K * m * m * 8 / 1e6, K * m * m * 4 / 1e6),
+    }
+
+
+def run_ours(args):
+    import torch
+    import paper_1602_01448_b200 as sharp
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU path (use --impl reference for the oracle)")
+    sharp.load_library()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    warm = max(args.warmup, 3)
+    main_ = measure(args, args.config, args.steps, warm, rank, world, dev, dist, not args.no_e2e, rank == 0)
+    # BASELINE.json's metric names m = 128 AND m = 256: the second headline size (config 4, full size) rides on the
+    # same line as `secondary` whenever the default workload (config 2) is benched
+    second = None
+    if args.config == 2 and not args.grid and not args.no_secondary:
+        second = measure(args, 4, max(1, min(args.steps, 3)), 3, rank, world, dev, dist, not args.no_e2e, rank == 0)
 
     if rank != 0:
         if dist is not None:
@@ -322,22 +375,25 @@ def run_ours(args):
         base, _, _ = time_oracle(args, steps=3, warmup=1)
         cpu = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
 
+    def block(r, config_number):
+        return {
+            "config": {"workload": r["workload"], "config_number": config_number, "l2": r["l2"],
+                       "parallelism": "independent scan per GPU, no collective" if world > 1 else "single GPU",
+                       "step": "set_object(flat) + iterate(iters, beta) + errors()"},
+            "value": r["value"], "unit": UNIT, "steps": r["steps"], "ms_per_step": r["ms"] / r["steps"],
+            "ms_per_iteration": r["ms"] / r["steps"] / r["iters"], "eps": r["eps"], "eps0": r["eps0"],
+            "gpu_launches": r["launches"], "clocks": r["clocks"], "roofline": r["roofline"], "e2e": r["e2e"],
+        }
+
+    m1 = block(main_, args.config)
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(cfg, iters), "config_number": args.config,
-                   "l2": "inputs larger than L2 (frame state 2x%.0f MB + amplitudes %.0f MB per iteration vs 126 MB L2)"
-                         % (K * m * m * 8 / 1e6, K * m * m * 4 / 1e6),
-                   "parallelism": "independent scan per GPU, no collective" if world > 1 else "single GPU",
-                   "step": "set_object(flat) + iterate(iters, beta) + errors()"},
-        "ms_per_iteration": ms / args.steps / iters,
-        "eps": [float(x) for x in eps],
-        "gpu_launches": int(launches),
-        "clocks": clocks,
-        "roofline": roofline,
-        "e2e": e2e,
-        "cpu_baseline": cpu,
+        "metric": METRIC, "value": m1["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": warm, "ms_per_step": m1["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": m1["config"],
+        "ms_per_iteration": m1["ms_per_iteration"], "eps": m1["eps"], "eps0": m1["eps0"],
+        "gpu_launches": m1["gpu_launches"] + (second["launches"] if second else 0),
+        "clocks": m1["clocks"], "roofline": m1["roofline"], "e2e": m1["e2e"], "cpu_baseline": cpu,
+        "secondary": block(second, 4) if second else None,
     }
     print(json.dumps(line), flush=True)
     if dist is not None:
