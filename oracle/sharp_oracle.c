@@ -16,12 +16,16 @@
  * serially in the stated order (ascending frame index i for sums over frames, reading G17).
  *
  * Readings of the paper used here (DESIGN.md section "Readings"): G1 RAAR sign, G2 DFT sign, G3 unitary
- * scaling, G4 small-|Fz| rule, G5 uncovered pixels, G7 z0, G10 step order when refining w.
+ * scaling, G4 small-|Fz| rule, G5 uncovered pixels, G7 z0, G10 step order when refining w, G21 default w0 at
+ * the frame centre, G22-G23 centre of mass of |w|^2 / integer cyclic shift of w alone, G24 small-|Fw| rule,
+ * G25 periodic T_i.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): DFT vs closed forms / Parseval / an independent library
  * FFT; Q,Q* adjointness; P_Q vs a dense matrix built from Eq. (5); projector idempotence; RAAR fixed point,
  * beta=1 Douglas-Rachford, literal vs one-overlap form; probe update closed forms; metric invariances;
- * tile lists vs interval arithmetic.  Parity unpinned: the absolute trajectory of the chaotic configs
+ * tile lists vs interval arithmetic; eps_0 vs a brute-force scan over phi and the expanded closed form; default
+ * probe returns a zero-phase pupil probe exactly; mask projection idempotent, |F w'| = a_w; re-centring moves a
+ * displaced probe back by the known integer; periodic T_i vs numpy.roll.  Parity unpinned: the absolute trajectory of the chaotic configs
  * beyond ~10 iterations.
  */
 #include <complex.h>
@@ -120,17 +124,26 @@ void orc_amplitudes(long n, const float *Iq, double *a, double *A2)
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * T_i: object pixel under frame pixel (r, c) of frame i.  PAPER.md:53 puts x_i in {0..n-m}, so r + x_i never
+ * leaves the image.  The simulation of PAPER.md:248 (Fig. 3) uses "periodic boundary conditions to avoid edge
+ * effects": x_i anywhere in {0..n-1} and r + x_i taken modulo the image size (reading G25).  The
+ * modulo below is the identity for positions in {0..n-m}, so both cases are this one expression.
+ * ---------------------------------------------------------------------------------------------- */
+static long obj_index(const int32_t *pos, int i, int r, int c, int nr, int nc)
+{
+    return (long)((pos[2 * i] + r) % nr) * nc + ((pos[2 * i + 1] + c) % nc);
+}
+
+/* ------------------------------------------------------------------------------------------------
  * O3  split: z_i(r) = w(r) psi(r + x_i)            PAPER.md:66-68 (Q_i = diag(w) T_i)
  * ---------------------------------------------------------------------------------------------- */
 void orc_split(int m, int K, const int32_t *pos, int nr, int nc, const cplx *psi, const cplx *w, cplx *z)
 {
-    (void)nr;
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < K; ++i)
         for (int r = 0; r < m; ++r)
             for (int c = 0; c < m; ++c)
-                z[((long)i * m + r) * m + c] =
-                    w[(long)r * m + c] * psi[(long)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + c)];
+                z[((long)i * m + r) * m + c] = w[(long)r * m + c] * psi[obj_index(pos, i, r, c, nr, nc)];
 }
 
 /* ------------------------------------------------------------------------------------------------
@@ -145,8 +158,7 @@ void orc_overlap_num(int m, int K, const int32_t *pos, int nr, int nc, const cpl
     for (int i = 0; i < K; ++i)
         for (int r = 0; r < m; ++r)
             for (int c = 0; c < m; ++c)
-                num[(long)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + c)] +=
-                    conj(w[(long)r * m + c]) * f[((long)i * m + r) * m + c];
+                num[obj_index(pos, i, r, c, nr, nc)] += conj(w[(long)r * m + c]) * f[((long)i * m + r) * m + c];
 }
 
 void orc_overlap_den(int m, int K, const int32_t *pos, int nr, int nc, const cplx *w, double *den)
@@ -156,8 +168,7 @@ void orc_overlap_den(int m, int K, const int32_t *pos, int nr, int nc, const cpl
         for (int r = 0; r < m; ++r)
             for (int c = 0; c < m; ++c) {
                 cplx wv = w[(long)r * m + c];
-                den[(long)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + c)] +=
-                    creal(wv) * creal(wv) + cimag(wv) * cimag(wv);
+                den[obj_index(pos, i, r, c, nr, nc)] += creal(wv) * creal(wv) + cimag(wv) * cimag(wv);
             }
 }
 
@@ -249,14 +260,13 @@ void orc_raar_one_split(int m, int K, const int32_t *pos, int nr, int nc, const 
  * ---------------------------------------------------------------------------------------------- */
 void orc_probe_update(int m, int K, const int32_t *pos, int nr, int nc, const cplx *psi, const cplx *z, cplx *w)
 {
-    (void)nr;
 #pragma omp parallel for schedule(static)
     for (int r = 0; r < m; ++r)
         for (int c = 0; c < m; ++c) {
             cplx num = 0.0;
             double den = 0.0;
             for (int i = 0; i < K; ++i) {
-                cplx pv = psi[(long)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + c)];
+                cplx pv = psi[obj_index(pos, i, r, c, nr, nc)];
                 num += conj(pv) * z[((long)i * m + r) * m + c];
                 den += creal(pv) * creal(pv) + cimag(pv) * cimag(pv);
             }
@@ -309,7 +319,7 @@ void orc_cover_counts(int m, int K, const int32_t *pos, int nr, int nc, int32_t 
     for (int i = 0; i < K; ++i)
         for (int r = 0; r < m; ++r)
             for (int c = 0; c < m; ++c)
-                count[(long)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + c)] += 1;
+                count[obj_index(pos, i, r, c, nr, nc)] += 1;
 }
 
 void orc_tile_lists(int m, int K, const int32_t *pos, int nr, int nc, int T, int32_t *tile_ptr, int32_t *frames)
@@ -327,4 +337,175 @@ void orc_tile_lists(int m, int K, const int32_t *pos, int nr, int nc, int T, int
             }
         }
     tile_ptr[ty_n * tx_n] = n;
+}
+
+/* Periodic versions of the integer artefacts (reading G25): the index of O10 (i) with the wrap of obj_index(),
+ * and the tile lists by brute force over PIXELS: frame i is in tile (ty,tx) iff one of its m x m pixels, taken
+ * modulo the image size, falls in the tile.  (Cover counts: orc_cover_counts already goes through obj_index().) */
+void orc_linear_index_periodic(int m, int K, const int32_t *pos, int nr, int nc, int64_t *idx)
+{
+    for (int i = 0; i < K; ++i)
+        for (int r = 0; r < m; ++r)
+            for (int c = 0; c < m; ++c) idx[((long)i * m + r) * m + c] = (int64_t)obj_index(pos, i, r, c, nr, nc);
+}
+
+void orc_tile_lists_periodic(int m, int K, const int32_t *pos, int nr, int nc, int T, int32_t *tile_ptr, int32_t *frames)
+{
+    int ty_n = (nr + T - 1) / T, tx_n = (nc + T - 1) / T;
+    int32_t n = 0;
+    for (int ty = 0; ty < ty_n; ++ty)
+        for (int tx = 0; tx < tx_n; ++tx) {
+            tile_ptr[ty * tx_n + tx] = n;
+            for (int i = 0; i < K; ++i) {
+                int hit_r = 0, hit_c = 0;
+                for (int r = 0; r < m; ++r) if ((pos[2 * i] + r) % nr / T == ty) hit_r = 1;
+                for (int c = 0; c < m; ++c) if ((pos[2 * i + 1] + c) % nc / T == tx) hit_c = 1;
+                if (hit_r && hit_c) { if (frames) frames[n] = i; ++n; }
+            }
+        }
+    tile_ptr[ty_n * tx_n] = n;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O11 error against a known solution, Eq. (14) PAPER.md:208-212:
+ *        eps_0(z) = min_phi || Q*(e^{i phi} z - z_0) || / || Q* z_0 ||,      z_0 = Q psi_0
+ *     Q* is the un-normalised overlap sum of O4 ("Notice the additional scaling factor Q*").  Q* uses the
+ *     illumination w; z_0 is formed with w0 (the illumination of the known solution; pass w0 = w when the
+ *     illumination is given).
+ *     With A = Q* z, B = Q* z_0:  || e^{i phi} A - B ||^2 = ||A||^2 + ||B||^2 - 2 Re(e^{i phi} <B, A>), <B,A> = sum conj(B) A,
+ *     which is smallest where e^{i phi} <B,A> is real and positive, i.e. phi* = -arg <B,A>.  The oracle takes that
+ *     phi* and then EVALUATES the norm of Eq. (14) literally at it (no expanded form); phi_out receives phi*.
+ *     tests/test_oracle_next.py checks the minimum against a brute-force scan over phi.
+ * ---------------------------------------------------------------------------------------------- */
+double orc_eps0(int m, int K, const int32_t *pos, int nr, int nc, const cplx *w, const cplx *w0, const cplx *z,
+                const cplx *psi0, double *phi_out)
+{
+    long N = (long)K * m * m, P = (long)nr * nc;
+    cplx *z0 = (cplx *)malloc(sizeof(cplx) * (size_t)N);
+    cplx *A = (cplx *)malloc(sizeof(cplx) * (size_t)P);
+    cplx *B = (cplx *)malloc(sizeof(cplx) * (size_t)P);
+    orc_split(m, K, pos, nr, nc, psi0, w0, z0);
+    orc_overlap_num(m, K, pos, nr, nc, w, z, A);
+    orc_overlap_num(m, K, pos, nr, nc, w, z0, B);
+    cplx ba = 0.0;
+    double nb = 0.0;
+    for (long p = 0; p < P; ++p) {
+        ba += conj(B[p]) * A[p];
+        nb += creal(B[p]) * creal(B[p]) + cimag(B[p]) * cimag(B[p]);
+    }
+    double phi = -carg(ba);
+    cplx e = cos(phi) + I * sin(phi);
+    double s = 0.0;
+    for (long p = 0; p < P; ++p) {
+        cplx d = e * A[p] - B[p];
+        s += creal(d) * creal(d) + cimag(d) * cimag(d);
+    }
+    free(z0); free(A); free(B);
+    if (phi_out) *phi_out = phi;
+    return sqrt(s / nb);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O12 default initialisations, PAPER.md:171-172 (steps 2-3).
+ *   step 2  "w0 = inverse Fourier transform of the square root of the average frame":
+ *             abar(q) = sqrt( (1/K) sum_i max(I_i(q), 0) ),   w0 = F* abar,
+ *           then moved to the frame centre by the cyclic shift (m/2, m/2) (reading G21: abar is real and
+ *           non-negative, so F* abar peaks at index (0,0); the illumination lives at the frame centre, PAPER.md:163,
+ *           reading G19).
+ *   step 3  "psi0 filled with random numbers uniformly drawn from [0,1)": the draw is a counter-based generator
+ *           that both sides implement (splitmix64 of seed and pixel index, top 24 bits -> float in [0,1)); real part
+ *           = the draw, imaginary part 0.  Compared BIT-EXACTLY with the library.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_default_probe(int m, int K, const float *Iq, cplx *w0)
+{
+    long mm = (long)m * m;
+    cplx *abar = (cplx *)malloc(sizeof(cplx) * (size_t)mm);
+    cplx *t = (cplx *)malloc(sizeof(cplx) * (size_t)mm);
+    for (long q = 0; q < mm; ++q) {
+        double s = 0.0;
+        for (int i = 0; i < K; ++i) {
+            double v = (double)Iq[(long)i * mm + q];
+            s += (v > 0.0) ? v : 0.0;
+        }
+        abar[q] = sqrt(s / (double)K);
+    }
+    orc_fft2(m, abar, t, +1);
+    for (int r = 0; r < m; ++r)
+        for (int c = 0; c < m; ++c) w0[(long)((r + m / 2) % m) * m + (c + m / 2) % m] = t[(long)r * m + c];
+    free(abar); free(t);
+}
+
+static uint64_t orc_splitmix64(uint64_t x)
+{
+    x += 0x9E3779B97F4A7C15ULL;
+    uint64_t z = x;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+void orc_random_object(long n, uint64_t seed, float *re)
+{
+    uint64_t k = orc_splitmix64(seed);
+    for (long p = 0; p < n; ++p) re[p] = (float)(orc_splitmix64(k + (uint64_t)p) >> 40) * (1.0f / 16777216.0f);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O13 illumination constraints, step 7 PAPER.md:181-189.
+ *   mask:       w <- F^{-1}{ (F w) m_w }                          m_w real (a support: 0/1, or any weights)
+ *   amplitude:  w <- F^{-1}{ (F w / |F w|) a_w }                  a_w = |F w_0| >= 0
+ *               where |F w| <= thr_w the phase factor is taken as 1, as in G4 (reading G24); the caller passes
+ *               thr_w = 1e-4 * rms(a_w).
+ *   Both m_w and a_w are indexed like the transform: DC at [0,0].
+ * ---------------------------------------------------------------------------------------------- */
+void orc_probe_mask(int m, const cplx *w, const double *mask, cplx *out)
+{
+    long mm = (long)m * m;
+    cplx *W = (cplx *)malloc(sizeof(cplx) * (size_t)mm);
+    orc_fft2(m, w, W, -1);
+    for (long q = 0; q < mm; ++q) W[q] *= mask[q];
+    orc_fft2(m, W, out, +1);
+    free(W);
+}
+
+void orc_probe_amplitude(int m, const cplx *w, const double *aw, double thr_w, cplx *out)
+{
+    long mm = (long)m * m;
+    cplx *W = (cplx *)malloc(sizeof(cplx) * (size_t)mm);
+    orc_fft2(m, w, W, -1);
+    for (long q = 0; q < mm; ++q) {
+        double mag = cabs(W[q]);
+        W[q] = (mag > thr_w) ? (W[q] / mag) * aw[q] : (cplx)aw[q];
+    }
+    orc_fft2(m, W, out, +1);
+    free(W);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O14 re-centring, PAPER.md:163 ("keeping the illumination in the center of the frame by computing the center of
+ *     mass and correcting for drifts after every update") and :191 ("compute center of mass of w and shift it").
+ *     Reading G22: the mass is |w|^2; the centre of mass is the plain first moment over the frame indices,
+ *         cm_r = sum r |w(r,c)|^2 / sum |w|^2   (likewise cm_c);
+ *     the shift is the INTEGER d = floor(m/2 - cm + 1/2) per axis (positions are integer pixels; the paper
+ *     defines no interpolation), applied cyclically: w'(r) = w((r - d) mod m).  Only w moves (reading G23).
+ *     d_out receives (d_r, d_c).  With sum |w|^2 = 0 nothing moves.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_probe_recentre(int m, const cplx *w, cplx *out, int32_t d_out[2])
+{
+    double s = 0.0, sr = 0.0, sc = 0.0;
+    for (int r = 0; r < m; ++r)
+        for (int c = 0; c < m; ++c) {
+            cplx v = w[(long)r * m + c];
+            double p = creal(v) * creal(v) + cimag(v) * cimag(v);
+            s += p; sr += p * r; sc += p * c;
+        }
+    int dr = 0, dc = 0;
+    if (s > 0.0) {
+        dr = (int)floor((double)(m / 2) - sr / s + 0.5);
+        dc = (int)floor((double)(m / 2) - sc / s + 0.5);
+    }
+    for (int r = 0; r < m; ++r)
+        for (int c = 0; c < m; ++c)
+            out[(long)(((r + dr) % m + m) % m) * m + ((c + dc) % m + m) % m] = w[(long)r * m + c];
+    d_out[0] = dr; d_out[1] = dc;
 }

@@ -11,6 +11,7 @@ marshals numpy arrays and strings the steps together in the paper's order:
   step 5  z  <- RAAR(z)                                PAPER.md:174-178  (sign: DESIGN.md reading G1)
   step 6  psi <- Q* z / Q* Q                           PAPER.md:180, Eq. (9)
   step 7  w  <- Eq. (10) every `refine_every` its      PAPER.md:181       (order: reading G10)
+          then the Fourier mask or amplitude constraint and the centre-of-mass shift (:191)
 
 Parity unpinned: see the header of sharp_oracle.c.
 """
@@ -204,13 +205,18 @@ class Oracle:
     """State (z, w, psi) advanced by steps 5-7 of PAPER.md:174-181.  Inputs are the same f32/c64 arrays the
     GPU library receives, widened to double once."""
 
-    def __init__(self, m, pos, shape, intensities, probe, psi0=None, refine_every=0):
+    def __init__(self, m, pos, shape, intensities, probe, psi0=None, refine_every=0, probe_mask=None,
+                 probe_amplitude=None, recentre=False):
         self.m = int(m); self.pos = _pos(pos); self.shape = tuple(int(s) for s in shape)
         self.K = self.pos.shape[0]
         I = np.asarray(intensities, dtype=np.float32).reshape(self.K, self.m, self.m)
         self.a, self.A2, self.a_rms, self.thr = amplitudes(I)
         self.w = _c(np.asarray(probe).reshape(self.m, self.m))
         self.refine_every = int(refine_every)
+        self.mask = None if probe_mask is None else np.asarray(probe_mask, dtype=np.float64)    # m_w  PAPER.md:181-185
+        self.aw = None if probe_amplitude is None else np.asarray(probe_amplitude, dtype=np.float64)   # a_w
+        self.recentre = bool(recentre)                                               # PAPER.md:191
+        self.shifts = []
         psi0 = np.ones(self.shape, np.complex128) if psi0 is None else _c(psi0)   # G8: flat 1+0i
         self.z = split(psi0, self.w, self.pos)                                      # step 4 (G7)
         self.zprev = None                                                           # "z^(0) = 0" for eps_Delta
@@ -231,11 +237,91 @@ class Oracle:
             self.psi = L(self.z, self.w, self.pos, self.shape)                              # step 6
             if self.refine_every and self.it % self.refine_every == 0:                      # step 7
                 self.w = probe_update(self.psi, self.z, self.w, self.pos)
+                if self.mask is not None:                                                   # "If m_w is given ..."
+                    self.w = probe_mask(self.w, self.mask)
+                elif self.aw is not None:                                                   # "else if a_w is given ..."
+                    self.w = probe_amplitude(self.w, self.aw)
+                if self.recentre:                                                           # "Now compute center of mass"
+                    self.w, d = probe_recentre(self.w)
+                    self.shifts.append(d)
         return self
 
     def object(self):
         """psi = L_w z with the current w (what sharp_get_object returns)."""
         return L(self.z, self.w, self.pos, self.shape)
 
+    def eps0(self, psi0, w0=None):
+        """Eq. (14) at the current frames, against the known solution psi0 (and its illumination w0)."""
+        return eps0(self.z, psi0, self.w, self.pos, self.shape, w0=w0)
+
     def errors(self):
         return errors(self.z, self.zprev, self.w, self.pos, self.shape, self.a, self.thr, self.A2)
+
+
+# ---- O11-O14: eps_0, default initialisations, illumination constraints, re-centring ---------------------------
+def eps0(z, psi0, w, pos, shape, w0=None, return_phi=False):
+    """Eq. (14): min_phi ||Q*(e^{i phi} z - z0)|| / ||Q* z0||, z0 = Q_{w0} psi0 (w0 = w if None)."""
+    z = _c(z); w = _c(w); w0 = w if w0 is None else _c(w0); psi0 = _c(psi0); pos = _pos(pos)
+    K, m, _ = z.shape; nr, nc = shape
+    phi = C.c_double(0.0)
+    f = lib().orc_eps0; f.restype = C.c_double
+    e = f(C.c_int(m), C.c_int(K), _p(pos), C.c_int(nr), C.c_int(nc), _p(w), _p(w0), _p(z), _p(psi0), C.byref(phi))
+    return (float(e), phi.value) if return_phi else float(e)
+
+
+def default_probe(I):
+    """PAPER.md:171 step 2: w0 = F*(sqrt(mean frame)), moved to the frame centre (reading G21)."""
+    I = np.ascontiguousarray(I, dtype=np.float32); K, m, _ = I.shape
+    w0 = np.empty((m, m), dtype=np.complex128)
+    lib().orc_default_probe(C.c_int(m), C.c_int(K), _p(I), _p(w0))
+    return w0
+
+
+def random_object(shape, seed):
+    """PAPER.md:172 step 3: psi0 ~ U[0,1) from the counter-based generator both sides implement (float32, exact)."""
+    nr, nc = shape
+    re = np.empty((nr, nc), dtype=np.float32)
+    lib().orc_random_object(C.c_long(nr * nc), C.c_uint64(seed), _p(re))
+    return re.astype(np.complex128)
+
+
+def probe_mask(w, mask):
+    w = _c(w); m = w.shape[0]; mask = np.ascontiguousarray(mask, dtype=np.float64)
+    out = np.empty_like(w)
+    lib().orc_probe_mask(C.c_int(m), _p(w), _p(mask), _p(out))
+    return out
+
+
+def probe_amplitude(w, aw, thr_w=None):
+    w = _c(w); m = w.shape[0]; aw = np.ascontiguousarray(aw, dtype=np.float64)
+    if thr_w is None:
+        thr_w = TAU * float(np.sqrt(np.mean(aw * aw)))           # reading G24
+    out = np.empty_like(w)
+    lib().orc_probe_amplitude(C.c_int(m), _p(w), _p(aw), C.c_double(thr_w), _p(out))
+    return out
+
+
+def probe_recentre(w):
+    w = _c(w); m = w.shape[0]
+    out = np.empty_like(w)
+    d = (C.c_int32 * 2)()
+    lib().orc_probe_recentre(C.c_int(m), _p(w), _p(out), d)
+    return out, (int(d[0]), int(d[1]))
+
+
+def linear_index_periodic(m, pos, shape):
+    pos = _pos(pos); K = pos.shape[0]; nr, nc = shape
+    idx = np.empty((K, m, m), dtype=np.int64)
+    lib().orc_linear_index_periodic(C.c_int(m), C.c_int(K), _p(pos), C.c_int(nr), C.c_int(nc), _p(idx))
+    return idx
+
+
+def tile_lists_periodic(m, pos, shape, T):
+    pos = _pos(pos); K = pos.shape[0]; nr, nc = shape
+    nt = ((nr + T - 1) // T) * ((nc + T - 1) // T)
+    ptr = np.empty(nt + 1, dtype=np.int32)
+    a = (C.c_int(m), C.c_int(K), _p(pos), C.c_int(nr), C.c_int(nc), C.c_int(T))
+    lib().orc_tile_lists_periodic(*a, _p(ptr), None)
+    frames = np.empty(int(ptr[-1]), dtype=np.int32)
+    lib().orc_tile_lists_periodic(*a, _p(ptr), _p(frames))
+    return ptr, frames
