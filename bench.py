@@ -299,8 +299,10 @@ def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e
         try:
             with open(traffic_file) as f:
                 t = json.load(f)
-            roofline["traffic"] = t.get("frame_kernel_dram_bytes_per_launch")
-            roofline["traffic_source"] = t.get("source")
+            # the capture may hold fewer frames per launch than this workload (config 4 is captured on a 40 x 40
+            # sub-raster): DRAM bytes per frame x the frames of this launch
+            roofline["traffic"] = int(t["frame_kernel_dram_bytes_per_frame"] * K)
+            roofline["traffic_source"] = t.get("source") + f"; {t['frames_per_launch_in_capture']} frames per launch in the capture, scaled to {K}"
         except Exception:
             pass
 

@@ -6,7 +6,7 @@
  *   P_a (Eq. 7), the overlap Q* / Q*Q (Eq. 8-9), the RAAR frame update
  *   (step 5), the optional illumination refinement (Eq. 10) and the
  *   residuals eps_a, eps_Q, eps_Delta (Eq. 11-13).
- * Readings of the paper where it is silent or garbled are listed in DESIGN.md ("Readings", G1..G20).
+ * Readings of the paper where it is silent or garbled are listed in DESIGN.md ("Readings", G1..G25).
  *
  * Conventions (all calls)
  *   - Arrays are row-major, C-contiguous.  Complex values are interleaved (re, im) float32 ("c64").
@@ -20,7 +20,8 @@
  *   - DFT convention: forward kernel exp(-2 pi i (u r + v c)/m), scale 1/m per 2-D transform each way
  *     (unitary; sign: reading G2); DC at index [0,0], no fftshift anywhere.
  *   - Positions x_i are the (row, col) of the frame's top-left pixel in the object, T_i psi(r) = psi(r + x_i)
- *     (PAPER.md:53, 68); 0 <= x_i <= obj - m on both axes, anything else is SHARP_EINVAL (no wrap-around).
+ *     (PAPER.md:53, 68); 0 <= x_i <= obj - m on both axes, anything else is SHARP_EINVAL (no wrap-around, except in a
+ *     plan made by sharp_plan_periodic).
  */
 #ifndef SHARP_B200_H
 #define SHARP_B200_H
@@ -55,6 +56,12 @@ typedef struct sharp_plan_s sharp_plan_t;
  *   obj_rows, obj_cols   object dimensions n_r x n_c, each >= m
  * No device work is done. */
 int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_rows, int obj_cols);
+/* sharp_plan_periodic: the same with the periodic boundary of the paper's Fig. 3 simulation ("periodic
+ * boundary conditions to avoid edge effects"; reading G25): T_i psi(r) = psi((r + x_i) mod n) on both axes, positions
+ * anywhere in 0 <= x_i < obj, and every frame-pixel <-> object-pixel map of the library (split, overlap, tile lists,
+ * cover counts, Eq. 10, residuals) wraps accordingly.  Requires obj - m >= SHARP_TILE - 1 on both axes (so that no
+ * object tile meets both ends of one frame); otherwise SHARP_EINVAL.  Everything else is as for sharp_plan. */
+int sharp_plan_periodic(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_rows, int obj_cols);
 void sharp_destroy(sharp_plan_t *p);
 /* Text of the last error on this plan (or of the last failed sharp_plan if p == NULL). Never NULL. */
 const char *sharp_last_error(const sharp_plan_t *p);
@@ -153,6 +160,40 @@ int sharp_op_overlap(sharp_plan_t *p, const float *f_dev, float *out_dev);
 int sharp_op_pa(sharp_plan_t *p, const float *f_dev, float *out_dev);
 int sharp_op_fft2(sharp_plan_t *p, const float *f_dev, float *out_dev, int sign);
 int sharp_op_probe(sharp_plan_t *p, const float *psi_dev, const float *z_dev, float *out_dev);
+
+/* ---- known-solution error and default initialisations ------------------------
+ * sharp_eps0: out HOST float <- eps_0 of Eq. (14), PAPER.md:208-212:
+ *      eps_0(z) = min_phi || Q*(e^{i phi} z - z_0) || / || Q* z_0 ||,     z_0 = Q_{w0} psi_0,
+ * at the current frames z, with Q* the un-normalised overlap sum under the CURRENT illumination.  psi0_dev: DEVICE
+ * obj c64, the known solution.  w0_dev: DEVICE m*m c64, the illumination of the known solution, or NULL when it is
+ * the plan's current illumination (the case of PAPER.md:248, "the exact illumination was given").  The minimum over
+ * the global phase is taken in closed form.  Does not change the state.  Synchronises.
+ * sharp_init_probe: step 2: installs w = F*( sqrt(average frame) ), moved to the frame centre by the
+ * cyclic shift (m/2, m/2) (reading G21), exactly as sharp_set_probe would.  Needs the intensities.
+ * sharp_init_object_random: step 3: psi^0 ~ U[0,1) (real), z^0 = Q psi^0.  The draw is counter-based:
+ * psi^0[p] = float(splitmix64(splitmix64(seed) + p) >> 40) / 2^24 for the row-major pixel index p.  Needs the probe.
+ * sharp_op_random_object: out_dev DEVICE obj c64 <- that psi^0 (test hook; state untouched). */
+int sharp_eps0(sharp_plan_t *p, const float *psi0_dev, const float *w0_dev, float *out_host);
+int sharp_init_probe(sharp_plan_t *p);
+int sharp_init_object_random(sharp_plan_t *p, unsigned long long seed);
+int sharp_op_random_object(sharp_plan_t *p, unsigned long long seed, float *out_dev);
+
+/* ---- illumination constraints and re-centring (step 7) -------
+ * Applied after every illumination update of Eq. 10 inside sharp_iterate, in the paper's order:
+ *   kind 1 (mask)       w <- F^{-1}{ (F w) m_w }
+ *   kind 2 (amplitude)  w <- F^{-1}{ (F w / |F w|) a_w };  where |F w| <= 1e-4 rms(a_w) the phase is taken as 1 (G24)
+ *   kind 0              unconstrained
+ * then, if re-centring is on: centre of mass of |w|^2 over the frame indices, integer shift
+ * d = floor(m/2 - cm + 1/2) per axis applied cyclically to w alone (readings G22, G23).
+ * con_dev: DEVICE m*m float32 indexed like the transform (DC at [0,0]); copied.  Ignored for kind 0.
+ * sharp_get_probe_shift: HOST int32[2] each: the last shift (d_r, d_c) and the sum of all shifts since
+ * sharp_set_probe_recentre was called; either may be NULL.  Synchronises.
+ * sharp_op_probe_constrain: out_dev[m*m c64] <- the configured constraint + re-centring applied to w_dev (test hook;
+ * out of place; records the shift, leaves the reconstruction state alone). */
+int sharp_set_probe_constraint(sharp_plan_t *p, int kind, const float *con_dev);
+int sharp_set_probe_recentre(sharp_plan_t *p, int on);
+int sharp_get_probe_shift(sharp_plan_t *p, int32_t last[2], int32_t total[2]);
+int sharp_op_probe_constrain(sharp_plan_t *p, const float *w_dev, float *out_dev);
 
 /* ---- host-buffer convenience (the end-to-end path bench.py times) -----------------------------------------
  * sharp_reconstruct_host: everything from HOST buffers: uploads I (K*m*m f32) and w (m*m c64), runs n

@@ -22,6 +22,7 @@ TILE = 32
 _vp, _i, _f, _sz, _ll = C.c_void_p, C.c_int, C.c_float, C.c_size_t, C.c_longlong
 _SIGNATURES = {
     "sharp_plan": (_i, [C.POINTER(_vp), _i, _i, _vp, _i, _i]),
+    "sharp_plan_periodic": (_i, [C.POINTER(_vp), _i, _i, _vp, _i, _i]),
     "sharp_destroy": (None, [_vp]),
     "sharp_last_error": (C.c_char_p, [_vp]),
     "sharp_workspace_bytes": (_sz, [_vp]),
@@ -51,6 +52,14 @@ _SIGNATURES = {
     "sharp_op_pa": (_i, [_vp, _vp, _vp]),
     "sharp_op_fft2": (_i, [_vp, _vp, _vp, _i]),
     "sharp_op_probe": (_i, [_vp, _vp, _vp, _vp]),
+    "sharp_eps0": (_i, [_vp, _vp, _vp, C.POINTER(_f)]),
+    "sharp_init_probe": (_i, [_vp]),
+    "sharp_init_object_random": (_i, [_vp, C.c_ulonglong]),
+    "sharp_op_random_object": (_i, [_vp, C.c_ulonglong, _vp]),
+    "sharp_set_probe_constraint": (_i, [_vp, _i, _vp]),
+    "sharp_set_probe_recentre": (_i, [_vp, _i]),
+    "sharp_get_probe_shift": (_i, [_vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]),
+    "sharp_op_probe_constrain": (_i, [_vp, _vp, _vp]),
     "sharp_reconstruct_host": (_i, [_vp, _vp, _vp, _i, _f, _vp, _vp, C.POINTER(_f)]),
 }
 
@@ -90,7 +99,7 @@ class Reconstruction:
     """One plan bound to one torch device/stream.  Methods have the names of the C calls without the prefix.
     Array arguments may be numpy arrays or torch tensors; they are moved to the device as float32 / complex64."""
 
-    def __init__(self, m, positions, obj_shape, device="cuda:0", stream=None):
+    def __init__(self, m, positions, obj_shape, device="cuda:0", stream=None, periodic=False):
         import torch
         self._torch = torch
         self.lib = load_library()
@@ -101,7 +110,9 @@ class Reconstruction:
         self.K = int(pos.shape[0])
         self.shape = (int(obj_shape[0]), int(obj_shape[1]))
         self._plan = C.c_void_p(None)
-        rc = self.lib.sharp_plan(C.byref(self._plan), self.m, self.K, pos.ctypes.data_as(C.c_void_p), *self.shape)
+        self.periodic = bool(periodic)
+        plan_fn = self.lib.sharp_plan_periodic if self.periodic else self.lib.sharp_plan
+        rc = plan_fn(C.byref(self._plan), self.m, self.K, pos.ctypes.data_as(C.c_void_p), *self.shape)
         if rc != SHARP_OK:
             raise SharpError(rc, self.lib.sharp_last_error(None).decode())
         self.device = torch.device(device) if device is not None else None
@@ -281,6 +292,46 @@ class Reconstruction:
         tz = self._dev(z, self._torch.complex64)
         out = self._new((self.m, self.m), self._torch.complex64)
         self._check(self.lib.sharp_op_probe(self._plan, _ptr(tp), _ptr(tz), _ptr(out)))
+        return out
+
+    # known-solution error, default initialisations, illumination constraints
+    def eps0(self, psi0, w0=None):
+        tp = self._dev(psi0, self._torch.complex64)
+        tw = self._dev(w0, self._torch.complex64)
+        assert tp.numel() == self.shape[0] * self.shape[1] and (tw is None or tw.numel() == self.m * self.m)
+        out = _f(0.0)
+        self._check(self.lib.sharp_eps0(self._plan, _ptr(tp), _ptr(tw), C.byref(out)))
+        return float(out.value)
+
+    def init_probe(self):
+        self._check(self.lib.sharp_init_probe(self._plan))
+
+    def init_object_random(self, seed):
+        self._check(self.lib.sharp_init_object_random(self._plan, C.c_ulonglong(int(seed))))
+
+    def op_random_object(self, seed):
+        out = self._new(self.shape, self._torch.complex64)
+        self._check(self.lib.sharp_op_random_object(self._plan, C.c_ulonglong(int(seed)), _ptr(out)))
+        return out
+
+    def set_probe_constraint(self, kind, con=None):
+        kind = {"none": 0, "mask": 1, "amplitude": 2}.get(kind, kind)
+        t = self._dev(con, self._torch.float32)
+        assert t is None or t.numel() == self.m * self.m
+        self._check(self.lib.sharp_set_probe_constraint(self._plan, int(kind), _ptr(t)))
+
+    def set_probe_recentre(self, on):
+        self._check(self.lib.sharp_set_probe_recentre(self._plan, int(bool(on))))
+
+    def get_probe_shift(self):
+        last, total = (C.c_int32 * 2)(), (C.c_int32 * 2)()
+        self._check(self.lib.sharp_get_probe_shift(self._plan, last, total))
+        return (int(last[0]), int(last[1])), (int(total[0]), int(total[1]))
+
+    def op_probe_constrain(self, w):
+        t = self._dev(w, self._torch.complex64)
+        out = self._new((self.m, self.m), self._torch.complex64)
+        self._check(self.lib.sharp_op_probe_constrain(self._plan, _ptr(t), _ptr(out)))
         return out
 
     def reconstruct_host(self, I_host, w_host, n, beta, want_eps=True):

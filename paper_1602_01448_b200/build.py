@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsharp_b200.so")
 SOURCES = ["sharp_b200.cu"]
-HEADERS = ["fft_regs.cuh", "frame_common.cuh", "frame_r.cuh", "frame_s.cuh", "object_kernels.cuh", os.path.join("..", "..", "include", "sharp_b200.h")]
+HEADERS = ["fft_regs.cuh", "frame_common.cuh", "frame_r.cuh", "frame_s.cuh", "object_kernels.cuh", "probe_kernels.cuh", os.path.join("..", "..", "include", "sharp_b200.h")]
 
 
 def needs_build() -> bool:

@@ -26,7 +26,7 @@ struct FrameArgs {
     const int *pos;          // K x 2
     float2 *scratch;         // gridDim.x * m * m
     const DevScalars *sc;
-    int K, nc;
+    int K, nr, nc;           // frames, object rows / columns (nr: only the periodic wrap and FRAME_ERR need it)
     float bm;                // beta / m^2
     float om;                // 1 - 2 beta
     int conj_io;             // FRAME_FFT: conjugate input and output (gives F*)

@@ -206,7 +206,9 @@ struct RPass {
 
 #if defined(__CUDACC__)
 
-template <int M, int MODE>
+// WRAP: the object index r + x_i is taken modulo the image size (periodic boundary of the Fig. 3 simulation, reading G25);
+// a separate instantiation, so the plain kernel pays nothing for it.
+template <int M, int MODE, bool WRAP = false>
 __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(FrameArgs A)
 {
     using C = RCfg<M>;
@@ -298,11 +300,21 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
             if (use_w) {
                 const float2 *prow = A.psi_v + (size_t)(xr + r_lo) * A.nc + xc + col;
                 const size_t pstep = (size_t)NLO * A.nc;
+                int pcw = xc + col;                  // WRAP only
+                if (WRAP && pcw >= A.nc) pcw -= A.nc;
 #pragma unroll
                 for (int ch = 0; ch < 4; ++ch) {
                     float2 pv[8], wv[8];
 #pragma unroll
-                    for (int k = 0; k < 8; ++k) pv[k] = __ldg(prow + (size_t)(8 * ch + k) * pstep);
+                    for (int k = 0; k < 8; ++k) {
+                        if constexpr (WRAP) {
+                            int prw = xr + r_lo + NLO * (8 * ch + k);
+                            if (prw >= A.nr) prw -= A.nr;
+                            pv[k] = __ldg(A.psi_v + (size_t)prw * A.nc + pcw);
+                        } else {
+                            pv[k] = __ldg(prow + (size_t)(8 * ch + k) * pstep);
+                        }
+                    }
                     if (w_tmem) {
                         r_tmem_ld16(tw_addr + 16 * ch, wv);
                     } else {
@@ -318,7 +330,10 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
 #pragma unroll
                 for (int k = 0; k < 32; ++k) {
                     const int r = r_lo + NLO * k;
-                    const size_t op = (size_t)(xr + r) * A.nc + xc + col;
+                    int prw = xr + r, pcw = xc + col;      // modulo the image size (identity without the periodic boundary)
+                    if (prw >= A.nr) prw -= A.nr;
+                    if (pcw >= A.nc) pcw -= A.nc;
+                    const size_t op = (size_t)prw * A.nc + pcw;
                     const float2 d = csub(cmul(__ldg(A.w_cur + r * M + col), __ldg(A.psi_z + op)), v[k]);
                     sq += d.x * d.x + d.y * d.y;
                     float2 zp = make_float2(0.f, 0.f);

@@ -216,7 +216,8 @@ __device__ __forceinline__ void s_st_scratch(float2 *p, float2 v, unsigned long 
 }
 
 // Launched with cluster dimension CS; gridDim.x is a multiple of CS.  scratch: one m x m frame per cluster.
-template <int M, int NT_, int MODE, int CS>
+// WRAP: periodic object index (see frame_r.cuh).
+template <int M, int NT_, int MODE, int CS, bool WRAP = false>
 __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
 {
     using C = SCfg<M, NT_>;
@@ -265,11 +266,21 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
                     const float2 *prow = A.psi_v + (size_t)(xr + r_lo) * A.nc + xc + col;
                     const float2 *wrow = A.w_form + (size_t)r_lo * M + col;
                     const size_t pstep = (size_t)NLO * A.nc;
+                    int pcw = xc + col;              // WRAP only
+                    if (WRAP && pcw >= A.nc) pcw -= A.nc;
 #pragma unroll
                     for (int ch = 0; ch < 4; ++ch) {
                         float2 pv[8], wv[8];
 #pragma unroll
-                        for (int k = 0; k < 8; ++k) pv[k] = __ldg(prow + (size_t)(8 * ch + k) * pstep);
+                        for (int k = 0; k < 8; ++k) {
+                            if constexpr (WRAP) {
+                                int prw = xr + r_lo + NLO * (8 * ch + k);
+                                if (prw >= A.nr) prw -= A.nr;
+                                pv[k] = __ldg(A.psi_v + (size_t)prw * A.nc + pcw);
+                            } else {
+                                pv[k] = __ldg(prow + (size_t)(8 * ch + k) * pstep);
+                            }
+                        }
 #pragma unroll
                         for (int k = 0; k < 8; ++k) wv[k] = __ldg(wrow + (size_t)(8 * ch + k) * (NLO * M));
 #pragma unroll
@@ -281,7 +292,10 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
 #pragma unroll
                     for (int k = 0; k < 32; ++k) {
                         const int r = r_lo + NLO * k;
-                        const size_t op = (size_t)(xr + r) * A.nc + xc + col;
+                        int prw = xr + r, pcw = xc + col;   // modulo the image size (identity without the periodic boundary)
+                        if (prw >= A.nr) prw -= A.nr;
+                        if (pcw >= A.nc) pcw -= A.nc;
+                        const size_t op = (size_t)prw * A.nc + pcw;
                         const float2 d = csub(cmul(__ldg(A.w_cur + r * M + col), __ldg(A.psi_z + op)), v[k]);
                         sq += d.x * d.x + d.y * d.y;
                         float2 zp = make_float2(0.f, 0.f);

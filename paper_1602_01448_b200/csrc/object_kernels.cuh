@@ -10,12 +10,23 @@ namespace sharp {
 
 constexpr int TILE = 32;  // == SHARP_TILE
 
+// T_i: linear object index under frame pixel (r, c) of a frame at (xr, xc).  With the periodic boundary of the Fig. 3
+// simulation (reading G25) positions lie anywhere in the image and r + x_i is taken modulo its size;
+// for the positions of PAPER.md:53 (x_i <= n - m) the two corrections never fire.
+__device__ __forceinline__ size_t obj_index(int xr, int xc, int r, int c, int nr, int nc)
+{
+    int rr = xr + r, cc = xc + c;
+    if (rr >= nr) rr -= nr;
+    if (cc >= nc) cc -= nc;
+    return (size_t)rr * nc + cc;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // a1 split:  z_i(r) = w(r) psi(r + x_i).  One thread per two consecutive frame pixels of a
 // row: 128-bit loads of w and stores of z; psi is only 8-byte aligned (x_i.col is arbitrary) so it is read as
 // two 64-bit loads.  psi == NULL means the flat object 1 + 0i (reading G8).
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_split(int m, int K, const int *pos, int nc, const float2 *psi,
+__global__ void __launch_bounds__(256) k_split(int m, int K, const int *pos, int nr, int nc, const float2 *psi,
                                                 const float2 *w, float2 *z)
 {
     const size_t half = (size_t)m / 2;
@@ -28,9 +39,8 @@ __global__ void __launch_bounds__(256) k_split(int m, int K, const int *pos, int
         const float4 w2 = __ldg(reinterpret_cast<const float4 *>(w + (size_t)r * m + c));
         float2 p0 = make_float2(1.f, 0.f), p1 = p0;
         if (psi != nullptr) {
-            const float2 *pp = psi + (size_t)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + c);
-            p0 = __ldg(pp);
-            p1 = __ldg(pp + 1);
+            p0 = __ldg(psi + obj_index(pos[2 * i], pos[2 * i + 1], r, c, nr, nc));
+            p1 = __ldg(psi + obj_index(pos[2 * i], pos[2 * i + 1], r, c + 1, nr, nc));
         }
         const float2 z0 = cmul(make_float2(w2.x, w2.y), p0), z1 = cmul(make_float2(w2.z, w2.w), p1);
         __stcs(reinterpret_cast<float4 *>(z + ((size_t)i * m + r) * m + c), make_float4(z0.x, z0.y, z1.x, z1.y));
@@ -38,7 +48,7 @@ __global__ void __launch_bounds__(256) k_split(int m, int K, const int *pos, int
 }
 
 // z = c + w_form . T psi_v  (materialise the frames kept in factored form; sharp_get_frames)
-__global__ void __launch_bounds__(256) k_materialize(int m, int K, const int *pos, int nc, const float2 *c,
+__global__ void __launch_bounds__(256) k_materialize(int m, int K, const int *pos, int nr, int nc, const float2 *c,
                                                       const float2 *psi_v, const float2 *w, float2 *z)
 {
     const size_t per_frame = (size_t)m * m;
@@ -49,13 +59,13 @@ __global__ void __launch_bounds__(256) k_materialize(int m, int K, const int *po
         const int r = (int)(rem / m), col = (int)(rem % m);
         float2 v = __ldcs(c + g);
         if (psi_v != nullptr)
-            v = cadd(v, cmul(__ldg(w + rem), __ldg(psi_v + (size_t)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + col))));
+            v = cadd(v, cmul(__ldg(w + rem), __ldg(psi_v + obj_index(pos[2 * i], pos[2 * i + 1], r, col, nr, nc))));
         z[g] = v;
     }
 }
 
 // linear object index of frame pixel (i, r, c), with the same expression the kernels above use (O10 (i))
-__global__ void __launch_bounds__(256) k_frame_index(int m, int K, const int *pos, int nc, long long *idx)
+__global__ void __launch_bounds__(256) k_frame_index(int m, int K, const int *pos, int nr, int nc, long long *idx)
 {
     const size_t per_frame = (size_t)m * m;
     const size_t total = (size_t)K * per_frame;
@@ -63,7 +73,7 @@ __global__ void __launch_bounds__(256) k_frame_index(int m, int K, const int *po
         const int i = (int)(g / per_frame);
         const size_t rem = g - (size_t)i * per_frame;
         const int r = (int)(rem / m), col = (int)(rem % m);
-        idx[g] = (long long)((size_t)(pos[2 * i] + r) * nc + (pos[2 * i + 1] + col));
+        idx[g] = (long long)obj_index(pos[2 * i], pos[2 * i + 1], r, col, nr, nc);
     }
 }
 
@@ -161,6 +171,7 @@ enum OverlapMode : int { OV_DEN = 0, OV_L = 1, OV_ITER = 2, OV_REGATHER = 3 };
 
 struct OverlapArgs {
     int m, nr, nc, tiles_c;
+    int periodic;           // positions anywhere in the image, frames wrap around its edges (reading G25)
     const int *pos;
     const int *tile_ptr;
     const int *tile_frames;
@@ -206,9 +217,16 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
         __syncthreads();
         for (int j = threadIdx.x; j < n; j += blockDim.x) {
             const int fi = __ldg(A.tile_frames + base + j);
+            int xr = __ldg(A.pos + 2 * fi), xc = __ldg(A.pos + 2 * fi + 1);
+            if (A.periodic) {
+                // the copy of the frame (at x or at x - n) that meets this tile: a frame that starts beyond the tile
+                // reaches it by wrapping (the plan guarantees n - m >= TILE - 1, so never both)
+                if (xr > tr * TILE + TILE - 1) xr -= A.nr;
+                if (xc > tc * TILE + TILE - 1) xc -= A.nc;
+            }
             s_fi[j] = fi;
-            s_xr[j] = __ldg(A.pos + 2 * fi);
-            s_xc[j] = __ldg(A.pos + 2 * fi + 1);
+            s_xr[j] = xr;
+            s_xc[j] = xc;
         }
         __syncthreads();
         for (int e0 = 0; e0 < n; e0 += UNR) {
@@ -302,7 +320,7 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
 // a chunk of consecutive frames (ascending i) per probe pixel; k_probe_final adds the chunks in ascending order
 // and divides; where the denominator is 0 the old value is kept.
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_probe_partial(int m, int K, int chunk, const int *pos, int nc,
+__global__ void __launch_bounds__(256) k_probe_partial(int m, int K, int chunk, const int *pos, int nr, int nc,
                                                         const float2 *c, const float2 *psi_v, const float2 *w_form,
                                                         const float2 *psi, float2 *pnum, float *pden)
 {
@@ -313,7 +331,7 @@ __global__ void __launch_bounds__(256) k_probe_partial(int m, int K, int chunk, 
     float2 num = make_float2(0.f, 0.f);
     float den = 0.f;
     for (int i = i0; i < i1; ++i) {
-        const size_t op = (size_t)(__ldg(pos + 2 * i) + r) * nc + (__ldg(pos + 2 * i + 1) + col);
+        const size_t op = obj_index(__ldg(pos + 2 * i), __ldg(pos + 2 * i + 1), r, col, nr, nc);
         const float2 ps = __ldg(psi + op);
         float2 z = __ldcs(c + (size_t)i * m * m + pix);
         if (psi_v != nullptr) z = cadd(z, cmul(wf, __ldg(psi_v + op)));

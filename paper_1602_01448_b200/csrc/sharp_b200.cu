@@ -15,12 +15,14 @@
 #include "frame_r.cuh"
 #include "frame_s.cuh"
 #include "object_kernels.cuh"
+#include "probe_kernels.cuh"
 
 using namespace sharp;
 
 namespace {
 
 constexpr double kTau = 1e-4;  // reading G4: thr = tau * a_rms
+constexpr int kQuadBlocks = 1184;       // grid of the eps_0 reduction (8 blocks per SM on 148 SMs; any device works)
 constexpr int kMaxFrameSlots = 1024;   // upper bound on the persistent frame grid (sizes the error partials)
 thread_local std::string g_plan_error = "";
 
@@ -30,6 +32,7 @@ size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct sharp_plan_s {
     int m = 0, K = 0, nr = 0, nc = 0;
+    bool periodic = false;             // sharp_plan_periodic: frames wrap around the image edges (reading G25)
     int tiles_r = 0, tiles_c = 0;
     std::vector<int32_t> pos;          // K x 2
     std::vector<int32_t> tile_ptr;     // tiles + 1
@@ -54,7 +57,7 @@ struct sharp_plan_s {
     // workspace offsets
     size_t o_a = 0, o_c[2] = {0, 0}, o_psi_z = 0, o_psi_v[2] = {0, 0}, o_den = 0, o_cross = 0, o_w[4] = {0, 0, 0, 0}, o_scratch = 0,
            o_pos = 0, o_tile_ptr = 0, o_tile_frames = 0, o_partials = 0, o_err_partials = 0, o_err_sums = 0, o_pnum = 0,
-           o_pden = 0, o_scalars = 0, o_total = 0;
+           o_pden = 0, o_scalars = 0, o_wtmp[3] = {0, 0, 0}, o_wcon = 0, o_pscal = 0, o_quads = 0, o_quad_sum = 0, o_total = 0;
 
     // state
     bool have_I = false, have_probe = false, have_frames = false, have_prev = false;
@@ -63,6 +66,8 @@ struct sharp_plan_s {
     bool prev_psi_v_zero = true;
     int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
     int refine_every = 0;
+    int probe_constraint = 0;          // 0 none, 1 Fourier mask m_w, 2 Fourier amplitude a_w
+    bool probe_recentre = false;       // centre-of-mass shift after every illumination update
     long long it = 0;
     long long launches = 0;
 
@@ -175,23 +180,33 @@ cudaError_t launch_cluster(KernelT kern, int grid, int nt, int smem, int cs, cud
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
-template <int MODE>
-int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
+template <int MODE, bool WRAP>
+int frame_dispatch_w(sharp_plan_t *p, const FrameArgs &a, int grid)
 {
     ProfScope prof(p, MODE == FRAME_ITER ? SHARP_PROF_FRAME : SHARP_PROF_OTHER);
     switch (p->m) {
-    case 64: k_frame_r<64, MODE><<<grid, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, p->stream>>>(a); break;
-    case 128: k_frame_r<128, MODE><<<grid, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, p->stream>>>(a); break;
+    case 64: k_frame_r<64, MODE, WRAP><<<grid, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, p->stream>>>(a); break;
+    case 128: k_frame_r<128, MODE, WRAP><<<grid, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, p->stream>>>(a); break;
     case 256:
-        CK(launch_cluster(k_frame_s<256, kNT256, MODE, kCluster256>, grid, kNT256, SCfg<256, kNT256>::SMEM_BYTES, kCluster256, p->stream, a));
+        CK(launch_cluster(k_frame_s<256, kNT256, MODE, kCluster256, WRAP>, grid, kNT256, SCfg<256, kNT256>::SMEM_BYTES, kCluster256, p->stream, a));
         break;
     case 512:
-        CK(launch_cluster(k_frame_s<512, 256, MODE, kCluster512>, grid, 256, SCfg<512, 256>::SMEM_BYTES, kCluster512, p->stream, a));
+        CK(launch_cluster(k_frame_s<512, 256, MODE, kCluster512, WRAP>, grid, 256, SCfg<512, 256>::SMEM_BYTES, kCluster512, p->stream, a));
         break;
     default: return fail(p, SHARP_EINVAL, "unsupported frame size %d", p->m);
     }
     CK_LAUNCH("k_frame");
     return SHARP_OK;
+}
+
+// the periodic plan runs the WRAP instantiation of the modes that index the object (FRAME_FFT does not)
+template <int MODE>
+int frame_dispatch(sharp_plan_t *p, const FrameArgs &a, int grid)
+{
+    if constexpr (MODE != FRAME_FFT) {
+        if (p->periodic) return frame_dispatch_w<MODE, true>(p, a, grid);
+    }
+    return frame_dispatch_w<MODE, false>(p, a, grid);
 }
 
 // sets the shared-memory attribute and returns how many CTAs of the kernel can be resident on the device
@@ -214,14 +229,14 @@ cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int cs, int sms, int 
     return e;
 }
 
-template <int MODE>
+template <int MODE, bool WRAP>
 cudaError_t frame_prepare_m(int m, int sms, int *resident)
 {
     switch (m) {
-    case 64: return kernel_prepare(k_frame_r<64, MODE>, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, 1, sms, resident);
-    case 128: return kernel_prepare(k_frame_r<128, MODE>, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, 1, sms, resident);
-    case 256: return kernel_prepare(k_frame_s<256, kNT256, MODE, kCluster256>, kNT256, SCfg<256, kNT256>::SMEM_BYTES, kCluster256, sms, resident);
-    default: return kernel_prepare(k_frame_s<512, 256, MODE, kCluster512>, 256, SCfg<512, 256>::SMEM_BYTES, kCluster512, sms, resident);
+    case 64: return kernel_prepare(k_frame_r<64, MODE, WRAP>, RCfg<64>::NT, RCfg<64>::SMEM_BYTES, 1, sms, resident);
+    case 128: return kernel_prepare(k_frame_r<128, MODE, WRAP>, RCfg<128>::NT, RCfg<128>::SMEM_BYTES, 1, sms, resident);
+    case 256: return kernel_prepare(k_frame_s<256, kNT256, MODE, kCluster256, WRAP>, kNT256, SCfg<256, kNT256>::SMEM_BYTES, kCluster256, sms, resident);
+    default: return kernel_prepare(k_frame_s<512, 256, MODE, kCluster512, WRAP>, 256, SCfg<512, 256>::SMEM_BYTES, kCluster512, sms, resident);
     }
 }
 
@@ -234,6 +249,7 @@ FrameArgs base_frame_args(sharp_plan_t *p)
     a.scratch = p->dp<float2>(p->o_scratch);
     a.sc = p->dp<DevScalars>(p->o_scalars);
     a.K = p->K;
+    a.nr = p->nr;
     a.nc = p->nc;
     return a;
 }
@@ -243,6 +259,7 @@ OverlapArgs base_overlap_args(sharp_plan_t *p)
     OverlapArgs a;
     memset(&a, 0, sizeof a);
     a.m = p->m; a.nr = p->nr; a.nc = p->nc; a.tiles_c = p->tiles_c;
+    a.periodic = p->periodic ? 1 : 0;
     a.pos = p->dp<int>(p->o_pos);
     a.tile_ptr = p->dp<int>(p->o_tile_ptr);
     a.tile_frames = p->dp<int>(p->o_tile_frames);
@@ -321,12 +338,65 @@ int adopt_frames(sharp_plan_t *p)
     return regather_psi_z(p);
 }
 
+// one m x m transform, out of place, natural order, unitary: the fused frame kernel in FRAME_FFT mode with K = 1
+int fft_single(sharp_plan_t *p, const float2 *in, float2 *out, int sign)
+{
+    FrameArgs fa = base_frame_args(p);
+    fa.K = 1;
+    fa.c_in = in;
+    fa.c_out = out;
+    fa.conj_io = (sign == 1);
+    return frame_dispatch<FRAME_FFT>(p, fa, cluster_size(p->m));
+}
+
+// Step 7 after Eq. 10: Fourier mask or amplitude constraint, then the centre-of-mass shift.
+// src (m x m, one of the o_wtmp buffers or a caller buffer) -> dst; src is left unchanged.
+int constrain_probe(sharp_plan_t *p, const float2 *src, float2 *dst)
+{
+    const int mm = p->m * p->m;
+    const float2 *cur = src;
+    if (p->probe_constraint != 0) {
+        float2 *W = p->dp<float2>(p->o_wtmp[1]);
+        float2 *back = p->probe_recentre ? p->dp<float2>(p->o_wtmp[2]) : dst;
+        if (int rc = fft_single(p, cur, W, -1)) return rc;
+        k_probe_fourier<<<mm / 256, 256, 0, p->stream>>>(mm, p->probe_constraint, p->dp<float>(p->o_wcon), p->dp<ProbeScalars>(p->o_pscal), W);
+        CK_LAUNCH("k_probe_fourier");
+        if (int rc = fft_single(p, W, back, +1)) return rc;
+        cur = back;
+    }
+    if (p->probe_recentre) {
+        k_probe_moments<<<1, 256, 0, p->stream>>>(p->m, cur, p->dp<ProbeScalars>(p->o_pscal));
+        CK_LAUNCH("k_probe_moments");
+        k_cyclic_shift<<<mm / 256, 256, 0, p->stream>>>(p->m, cur, p->dp<ProbeScalars>(p->o_pscal)->shift, dst);
+        CK_LAUNCH("k_cyclic_shift");
+    } else if (cur != dst) {
+        CK(cudaMemcpyAsync(dst, cur, (size_t)mm * 8, cudaMemcpyDeviceToDevice, p->stream));
+    }
+    return SHARP_OK;
+}
+
 }  // namespace
 
-// =================================================================================================================
-extern "C" {
+namespace {
+// Tiles met by the pixels [x, x + m) of one axis, taken modulo n when the plan is periodic: at most two index ranges
+// [lo, hi] (the second one is the wrapped tail).  The periodic plan requires n - m >= TILE - 1, which keeps the two
+// ranges disjoint (no tile sees both ends of a frame).
+struct TileRanges { int n; int lo[2], hi[2]; };
+static TileRanges tile_ranges(int x, int m, int n)
+{
+    TileRanges t;
+    t.n = 1;
+    t.lo[0] = x / TILE;
+    t.hi[0] = (std::min(x + m, n) - 1) / TILE;
+    if (x + m > n) {
+        t.n = 2;
+        t.lo[1] = 0;
+        t.hi[1] = (x + m - n - 1) / TILE;
+    }
+    return t;
+}
 
-int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_rows, int obj_cols)
+static int make_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_rows, int obj_cols, bool periodic)
 {
     if (!out) return fail(nullptr, SHARP_EINVAL, "out is NULL");
     *out = nullptr;
@@ -334,38 +404,42 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     if (K < 1) return fail(nullptr, SHARP_EINVAL, "K must be >= 1 (got %d)", K);
     if (!pos_rc) return fail(nullptr, SHARP_EINVAL, "pos_rc is NULL");
     if (obj_rows < m || obj_cols < m) return fail(nullptr, SHARP_EINVAL, "object %d x %d smaller than the frame %d", obj_rows, obj_cols, m);
+    if (periodic && (obj_rows - m < TILE - 1 || obj_cols - m < TILE - 1))
+        return fail(nullptr, SHARP_EINVAL, "periodic plan: the object must exceed the frame by at least %d pixels per axis", TILE - 1);
     if ((long long)K * m * m > (1LL << 40) || (long long)obj_rows * obj_cols > (1LL << 31) - 1)
         return fail(nullptr, SHARP_EINVAL, "problem too large");
     for (int i = 0; i < K; ++i) {
         const int r = pos_rc[2 * i], c = pos_rc[2 * i + 1];
-        if (r < 0 || c < 0 || r > obj_rows - m || c > obj_cols - m)
-            return fail(nullptr, SHARP_EINVAL, "position %d = (%d, %d) outside [0, %d] x [0, %d] (PAPER.md:53)", i, r, c, obj_rows - m, obj_cols - m);
+        const int rmax = periodic ? obj_rows - 1 : obj_rows - m, cmax = periodic ? obj_cols - 1 : obj_cols - m;
+        if (r < 0 || c < 0 || r > rmax || c > cmax)
+            return fail(nullptr, SHARP_EINVAL, "position %d = (%d, %d) outside [0, %d] x [0, %d] (PAPER.md:53%s)", i, r, c, rmax, cmax,
+                        periodic ? "; periodic boundary, PAPER.md:248" : "");
     }
     sharp_plan_t *p = new (std::nothrow) sharp_plan_s;
     if (!p) return fail(nullptr, SHARP_ENOMEM, "host allocation failed");
     p->m = m; p->K = K; p->nr = obj_rows; p->nc = obj_cols;
+    p->periodic = periodic;
     p->pos.assign(pos_rc, pos_rc + 2 * (size_t)K);
     p->tiles_r = (obj_rows + TILE - 1) / TILE;
     p->tiles_c = (obj_cols + TILE - 1) / TILE;
 
-    // CSR tile lists by a two-pass counting sort over frames in ascending index: frame i touches the tile
-    // rectangle [r/T, (r+m-1)/T] x [c/T, (c+m-1)/T].
+    // CSR tile lists by a two-pass counting sort over frames in ascending index: frame i touches the tiles of
+    // tile_ranges(row) x tile_ranges(col).
     const size_t ntiles = (size_t)p->tiles_r * p->tiles_c;
     p->tile_ptr.assign(ntiles + 1, 0);
-    for (int i = 0; i < K; ++i) {
-        const int r = pos_rc[2 * i], c = pos_rc[2 * i + 1];
-        for (int ty = r / TILE; ty <= (r + m - 1) / TILE; ++ty)
-            for (int tx = c / TILE; tx <= (c + m - 1) / TILE; ++tx) ++p->tile_ptr[(size_t)ty * p->tiles_c + tx + 1];
-    }
+    auto for_each_tile = [&](int i, auto &&fn) {
+        const TileRanges tr = tile_ranges(pos_rc[2 * i], m, obj_rows), tc = tile_ranges(pos_rc[2 * i + 1], m, obj_cols);
+        for (int a = 0; a < tr.n; ++a)
+            for (int ty = tr.lo[a]; ty <= tr.hi[a]; ++ty)
+                for (int b = 0; b < tc.n; ++b)
+                    for (int tx = tc.lo[b]; tx <= tc.hi[b]; ++tx) fn((size_t)ty * p->tiles_c + tx);
+    };
+    for (int i = 0; i < K; ++i) for_each_tile(i, [&](size_t t) { ++p->tile_ptr[t + 1]; });
     for (size_t j = 0; j < ntiles; ++j) p->tile_ptr[j + 1] += p->tile_ptr[j];
     p->tile_frames.resize((size_t)p->tile_ptr[ntiles]);
     {
         std::vector<int32_t> fill(p->tile_ptr.begin(), p->tile_ptr.end() - 1);
-        for (int i = 0; i < K; ++i) {
-            const int r = pos_rc[2 * i], c = pos_rc[2 * i + 1];
-            for (int ty = r / TILE; ty <= (r + m - 1) / TILE; ++ty)
-                for (int tx = c / TILE; tx <= (c + m - 1) / TILE; ++tx) p->tile_frames[(size_t)fill[(size_t)ty * p->tiles_c + tx]++] = i;
-        }
+        for (int i = 0; i < K; ++i) for_each_tile(i, [&](size_t t) { p->tile_frames[(size_t)fill[t]++] = i; });
     }
 
     // workspace layout.  The frame kernel is persistent: at most one scratch slot per resident CTA.
@@ -397,9 +471,29 @@ int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_
     p->o_pnum = take((size_t)p->probe_nchunks * m * m * 8);
     p->o_pden = take((size_t)p->probe_nchunks * m * m * 4);
     p->o_scalars = take(sizeof(DevScalars));
+    for (int j = 0; j < 3; ++j) p->o_wtmp[j] = take((size_t)m * m * 8);
+    p->o_wcon = take((size_t)m * m * 4);
+    p->o_pscal = take(sizeof(ProbeScalars));
+    p->o_quads = take((size_t)kQuadBlocks * 4 * 8);
+    p->o_quad_sum = take(4 * 8);
     p->o_total = o;
     *out = p;
     return SHARP_OK;
+}
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+int sharp_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_rows, int obj_cols)
+{
+    return make_plan(out, m, K, pos_rc, obj_rows, obj_cols, false);
+}
+
+int sharp_plan_periodic(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, int obj_rows, int obj_cols)
+{
+    return make_plan(out, m, K, pos_rc, obj_rows, obj_cols, true);
 }
 
 void sharp_destroy(sharp_plan_t *p)
@@ -430,10 +524,12 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     int resident = 0, resident2 = 0;
-    CK(frame_prepare_m<FRAME_ITER>(p->m, sms, &resident));
-    CK(frame_prepare_m<FRAME_FFT>(p->m, sms, &resident2));
+    if (p->periodic) CK((frame_prepare_m<FRAME_ITER, true>(p->m, sms, &resident)));
+    else CK((frame_prepare_m<FRAME_ITER, false>(p->m, sms, &resident)));
+    CK((frame_prepare_m<FRAME_FFT, false>(p->m, sms, &resident2)));
     resident = std::min(resident, resident2);
-    CK(frame_prepare_m<FRAME_ERR>(p->m, sms, &resident2));
+    if (p->periodic) CK((frame_prepare_m<FRAME_ERR, true>(p->m, sms, &resident2)));
+    else CK((frame_prepare_m<FRAME_ERR, false>(p->m, sms, &resident2)));
     resident = std::min(resident, resident2);
     if (resident < 1) return fail(p, SHARP_ECUDA, "frame kernel does not fit on the device");
     p->sms = sms;
@@ -445,6 +541,7 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     if (!p->tile_frames.empty())
         CK(cudaMemcpyAsync(p->dp<int>(p->o_tile_frames), p->tile_frames.data(), p->tile_frames.size() * 4, cudaMemcpyHostToDevice, p->stream));
     CK(cudaMemsetAsync(p->dp<void>(p->o_scalars), 0, sizeof(DevScalars), p->stream));
+    CK(cudaMemsetAsync(p->dp<void>(p->o_pscal), 0, sizeof(ProbeScalars), p->stream));
     CK(cudaStreamSynchronize(p->stream));  // the host vectors may be read until here
     p->bound = true;
     p->have_I = p->have_probe = p->have_frames = p->have_prev = false;
@@ -490,7 +587,7 @@ int sharp_set_object(sharp_plan_t *p, const float *psi_dev)
 {
     if (int rc = check_ready(p, false, true)) return rc;
     p->cur = 0; p->vcur = 0;
-    k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc,
+    k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc,
                                                             reinterpret_cast<const float2 *>(psi_dev),
                                                             p->dp<float2>(p->o_w[p->w_cur]), p->dp<float2>(p->o_c[0]));
     CK_LAUNCH("k_split");
@@ -564,7 +661,7 @@ int sharp_iterate(sharp_plan_t *p, int n, float beta)
             dim3 g(mm_i / 256, p->probe_nchunks);
             {
                 ProfScope prof(p, SHARP_PROF_PROBE);
-                k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nc,
+                k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nr, p->nc,
                                                           p->dp<float2>(p->o_c[p->cur]), p->dp<float2>(p->o_psi_v[p->vcur]),
                                                           p->dp<float2>(p->o_w[p->w_form]), p->dp<float2>(p->o_psi_z),
                                                           p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden));
@@ -572,9 +669,13 @@ int sharp_iterate(sharp_plan_t *p, int n, float beta)
             CK_LAUNCH("k_probe_partial");
             int slot = free_probe_slot(p);
             if (slot < 0) return fail(p, SHARP_ECUDA, "internal: no free probe slot");
+            const bool post = p->probe_constraint != 0 || p->probe_recentre;
+            float2 *w_eq10 = post ? p->dp<float2>(p->o_wtmp[0]) : p->dp<float2>(p->o_w[slot]);
             k_probe_final<<<mm_i / 256, 256, 0, p->stream>>>(p->m, p->probe_nchunks, p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden),
-                                                             p->dp<float2>(p->o_w[p->w_cur]), p->dp<float2>(p->o_w[slot]));
+                                                             p->dp<float2>(p->o_w[p->w_cur]), w_eq10);
             CK_LAUNCH("k_probe_final");
+            if (post)
+                if (int rc = constrain_probe(p, w_eq10, p->dp<float2>(p->o_w[slot]))) return rc;
             p->w_cur = slot;
             if (int rc = rebuild_den(p)) return rc;
             if (int rc = regather_psi_z(p)) return rc;
@@ -605,7 +706,7 @@ int sharp_get_frames(sharp_plan_t *p, float *out_dev)
     if (int rc = check_ready(p, false, true)) return rc;
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
-    k_materialize<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc, p->dp<float2>(p->o_c[p->cur]),
+    k_materialize<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc, p->dp<float2>(p->o_c[p->cur]),
                                                              p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]),
                                                              p->dp<float2>(p->o_w[p->w_form]), reinterpret_cast<float2 *>(out_dev));
     CK_LAUNCH("k_materialize");
@@ -704,13 +805,17 @@ int sharp_tile_lists(const sharp_plan_t *p, const int32_t **tile_ptr, const int3
 int sharp_cover_counts(const sharp_plan_t *p, int32_t *out_host)
 {
     if (!p || !out_host) return SHARP_EINVAL;
-    // 2-D difference array: +1/-1 at the corners of every frame, then prefix sums along both axes
+    // 2-D difference array: +1/-1 at the corners of every rectangle, then prefix sums along both axes; a frame that
+    // wraps around an edge of a periodic plan is up to four rectangles
     const int nr = p->nr, nc = p->nc, m = p->m;
     std::vector<int32_t> d((size_t)(nr + 1) * (nc + 1), 0);
     auto at = [&](int r, int c) -> int32_t & { return d[(size_t)r * (nc + 1) + c]; };
+    auto rect = [&](int r0, int r1, int c0, int c1) { at(r0, c0) += 1; at(r0, c1) -= 1; at(r1, c0) -= 1; at(r1, c1) += 1; };
     for (int i = 0; i < p->K; ++i) {
         const int r = p->pos[2 * i], c = p->pos[2 * i + 1];
-        at(r, c) += 1; at(r, c + m) -= 1; at(r + m, c) -= 1; at(r + m, c + m) += 1;
+        const int rs[2][2] = {{r, std::min(r + m, nr)}, {0, r + m - nr}}, cs[2][2] = {{c, std::min(c + m, nc)}, {0, c + m - nc}};
+        for (int a = 0; a < (r + m > nr ? 2 : 1); ++a)
+            for (int b = 0; b < (c + m > nc ? 2 : 1); ++b) rect(rs[a][0], rs[a][1], cs[b][0], cs[b][1]);
     }
     for (int r = 0; r <= nr; ++r)
         for (int c = 1; c <= nc; ++c) at(r, c) += at(r, c - 1);
@@ -725,7 +830,7 @@ int sharp_frame_index(sharp_plan_t *p, long long *out_dev)
 {
     if (int rc = check_ready(p, false, false)) return rc;
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
-    k_frame_index<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc, out_dev);
+    k_frame_index<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc, out_dev);
     CK_LAUNCH("k_frame_index");
     return SHARP_OK;
 }
@@ -734,7 +839,7 @@ int sharp_op_split(sharp_plan_t *p, const float *psi_dev, float *out_dev)
 {
     if (int rc = check_ready(p, false, true)) return rc;
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
-    k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nc, reinterpret_cast<const float2 *>(psi_dev),
+    k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc, reinterpret_cast<const float2 *>(psi_dev),
                                                             p->dp<float2>(p->o_w[p->w_cur]), reinterpret_cast<float2 *>(out_dev));
     CK_LAUNCH("k_split");
     return SHARP_OK;
@@ -782,7 +887,7 @@ int sharp_op_probe(sharp_plan_t *p, const float *psi_dev, const float *z_dev, fl
     if (!psi_dev || !z_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
     const int mm_i = p->m * p->m;
     dim3 g(mm_i / 256, p->probe_nchunks);
-    k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nc,
+    k_probe_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<int>(p->o_pos), p->nr, p->nc,
                                               reinterpret_cast<const float2 *>(z_dev), nullptr, p->dp<float2>(p->o_w[p->w_cur]),
                                               reinterpret_cast<const float2 *>(psi_dev), p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden));
     CK_LAUNCH("k_probe_partial");
@@ -814,6 +919,111 @@ int sharp_reconstruct_host(sharp_plan_t *p, const float *I_host, const float *w_
     if (w_out_host) CK(cudaMemcpyAsync(w_out_host, p->dp<void>(p->o_w[p->w_cur]), (size_t)p->m * p->m * 8, cudaMemcpyDeviceToHost, p->stream));
     CK(cudaStreamSynchronize(p->stream));
     return SHARP_OK;
+}
+
+// ---- eps_0 against a known solution, default initialisations ----------------------------------
+int sharp_eps0(sharp_plan_t *p, const float *psi0_dev, const float *w0_dev, float *out_host)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    if (!psi0_dev || !out_host) return fail(p, SHARP_EINVAL, "NULL argument");
+    if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
+    const float2 *cross = nullptr;
+    if (w0_dev != nullptr) {
+        // B = Q* Q_{w0} psi_0 = psi_0 . sum_i conj(w) w0: the cross term the Q*Q kernel already knows how to build
+        OverlapArgs a = base_overlap_args(p);
+        a.w_a = p->dp<float2>(p->o_w[p->w_cur]);
+        a.w_b = reinterpret_cast<const float2 *>(w0_dev);
+        if (int rc = overlap_launch<OV_DEN>(p, a)) return rc;
+        cross = p->dp<float2>(p->o_cross);
+    }
+    k_eps0_partial<<<kQuadBlocks, 256, 0, p->stream>>>(p->nobj(), p->dp<float2>(p->o_psi_z), p->dp<float>(p->o_den),
+                                                       reinterpret_cast<const float2 *>(psi0_dev), cross, p->dp<double>(p->o_quads));
+    CK_LAUNCH("k_eps0_partial");
+    k_sum_quads<<<1, 32, 0, p->stream>>>(kQuadBlocks, p->dp<double>(p->o_quads), p->dp<double>(p->o_quad_sum));
+    CK_LAUNCH("k_sum_quads");
+    double q[4];
+    CK(cudaMemcpyAsync(q, p->dp<void>(p->o_quad_sum), sizeof q, cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+    const double d2 = q[0] + q[1] - 2.0 * sqrt(q[2] * q[2] + q[3] * q[3]);
+    *out_host = q[1] > 0.0 ? (float)sqrt(std::max(d2, 0.0) / q[1]) : 0.0f;
+    return SHARP_OK;
+}
+
+int sharp_init_probe(sharp_plan_t *p)
+{
+    if (int rc = check_ready(p, true, false)) return rc;
+    const int mm = p->m * p->m;
+    double *part = p->dp<double>(p->o_pnum);                // probe_nchunks * m * m * 8 bytes
+    dim3 g(mm / 256, p->probe_nchunks);
+    k_mean_frame_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<float>(p->o_a), part);
+    CK_LAUNCH("k_mean_frame_partial");
+    k_mean_frame_final<<<mm / 256, 256, 0, p->stream>>>(p->m, p->K, p->probe_nchunks, part, p->dp<float2>(p->o_wtmp[0]));
+    CK_LAUNCH("k_mean_frame_final");
+    if (int rc = fft_single(p, p->dp<float2>(p->o_wtmp[0]), p->dp<float2>(p->o_wtmp[1]), +1)) return rc;
+    k_cyclic_shift<<<mm / 256, 256, 0, p->stream>>>(p->m, p->dp<float2>(p->o_wtmp[1]), nullptr, p->dp<float2>(p->o_wtmp[2]));
+    CK_LAUNCH("k_cyclic_shift");
+    return sharp_set_probe(p, p->dp<float>(p->o_wtmp[2]));
+}
+
+int sharp_op_random_object(sharp_plan_t *p, unsigned long long seed, float *out_dev)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
+    k_random_object<<<grid_for(p->nobj()), 256, 0, p->stream>>>(p->nobj(), seed, reinterpret_cast<float2 *>(out_dev));
+    CK_LAUNCH("k_random_object");
+    return SHARP_OK;
+}
+
+int sharp_init_object_random(sharp_plan_t *p, unsigned long long seed)
+{
+    if (int rc = check_ready(p, false, true)) return rc;
+    // psi_v[1] is free here: sharp_set_object resets the factored state (psi_v = 0) before anything reads it
+    float *tmp = p->dp<float>(p->o_psi_v[1]);
+    if (int rc = sharp_op_random_object(p, seed, tmp)) return rc;
+    return sharp_set_object(p, tmp);
+}
+
+// ---- illumination constraints and re-centring --------------------------------------------------
+int sharp_set_probe_constraint(sharp_plan_t *p, int kind, const float *con_dev)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (kind < 0 || kind > 2) return fail(p, SHARP_EINVAL, "constraint kind must be 0 (none), 1 (mask) or 2 (amplitude)");
+    if (kind != 0 && !con_dev) return fail(p, SHARP_EINVAL, "con_dev is NULL");
+    const int mm = p->m * p->m;
+    if (kind != 0) {
+        CK(cudaMemcpyAsync(p->dp<void>(p->o_wcon), con_dev, (size_t)mm * 4, cudaMemcpyDeviceToDevice, p->stream));
+        k_constraint_scalars<<<1, 256, 0, p->stream>>>(mm, p->dp<float>(p->o_wcon), kTau, p->dp<ProbeScalars>(p->o_pscal));
+        CK_LAUNCH("k_constraint_scalars");
+    }
+    p->probe_constraint = kind;
+    return SHARP_OK;
+}
+
+int sharp_set_probe_recentre(sharp_plan_t *p, int on)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    p->probe_recentre = on != 0;
+    CK(cudaMemsetAsync(p->dp<ProbeScalars>(p->o_pscal)->shift, 0, 4 * sizeof(int), p->stream));
+    return SHARP_OK;
+}
+
+int sharp_get_probe_shift(sharp_plan_t *p, int32_t last[2], int32_t total[2])
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    ProbeScalars ps;
+    CK(cudaMemcpyAsync(&ps, p->dp<void>(p->o_pscal), sizeof ps, cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+    if (last) { last[0] = ps.shift[0]; last[1] = ps.shift[1]; }
+    if (total) { total[0] = ps.total[0]; total[1] = ps.total[1]; }
+    return SHARP_OK;
+}
+
+int sharp_op_probe_constrain(sharp_plan_t *p, const float *w_dev, float *out_dev)
+{
+    if (int rc = check_ready(p, false, false)) return rc;
+    if (!w_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
+    if (w_dev == out_dev) return fail(p, SHARP_EINVAL, "sharp_op_probe_constrain is out of place");
+    return constrain_probe(p, reinterpret_cast<const float2 *>(w_dev), reinterpret_cast<float2 *>(out_dev));
 }
 
 }  // extern "C"

@@ -96,6 +96,7 @@ class ScanConfig:
     seed: int
     blind_start: bool = False   # start probe = Gaussian sigma=m/8 (configs 3, 5)
     phase_coeff: float = 0.01   # pupil phase = phase_coeff * rho^2 (the configs say 0.01)
+    periodic: int = 0           # > 0: periodic boundary on a periodic x periodic image (the paper's Fig. 3 simulation)
 
     @property
     def K(self) -> int:
@@ -103,6 +104,8 @@ class ScanConfig:
 
     @property
     def shape(self):
+        if self.periodic:
+            return (self.periodic, self.periodic)
         if self.kind == "raster":
             n = (self.grid - 1) * self.step + self.m + 2 * self.jitter
             return (n, n)
@@ -124,11 +127,18 @@ def config(n: int) -> ScanConfig:
         return ScanConfig("large", 256, "raster", 100, 48, 6, 48.0, 0.0, 0.9, 100, 0, s)
     if n == 5:
         return ScanConfig("very-large", 512, "fermat", 1600, 48, 0, 96.0, 1e6, 0.75, 100, 1, s, True)
-    raise ValueError("config number must be 1..5")
+    if n == 6:
+        # the paper's own Fig. 3 shape: 10,000 frames 128x128 on a 1000x1000 image, periodic boundary,
+        # 164 frames per pixel, exact illumination given, noise-free; beta is the paper's default
+        return ScanConfig("fig3-periodic", 128, "raster", 100, 10, 0, 24.0, 0.0, 0.75, 100, 0, s, periodic=1000)
+    raise ValueError("config number must be 1..6")
 
 
 def reduced(cfg: ScanConfig, grid: int, **kw) -> ScanConfig:
-    """The same recipe on a smaller raster / fewer spiral points (sizes the oracle finishes in seconds)."""
+    """The same recipe on a smaller raster / fewer spiral points (sizes the oracle finishes in seconds).  A periodic
+    scan keeps its step and shrinks the image with the raster (grid * step pixels), so it still tiles the torus."""
+    if cfg.periodic and "periodic" not in kw:
+        kw["periodic"] = grid * cfg.step
     return replace(cfg, grid=grid, name=f"{cfg.name}-g{grid}", **kw)
 
 
@@ -193,6 +203,8 @@ def exit_waves(cfg: ScanConfig, obj: np.ndarray, probe: np.ndarray, pos: np.ndar
     r = np.arange(m)
     rows = pos[lo:hi, 0, None, None] + r[None, :, None]
     cols = pos[lo:hi, 1, None, None] + r[None, None, :]
+    if cfg.periodic:
+        rows, cols = rows % obj.shape[0], cols % obj.shape[1]
     return probe.astype(np.complex128)[None] * obj.astype(np.complex128)[rows, cols]
 
 

@@ -75,3 +75,39 @@ def test_tile_lists_and_cover_counts_bit_exact(lib, oracle, case):
     ocnt = oracle.cover_counts(m, pos, shape)
     assert np.array_equal(cnt, ocnt) and int(cnt.sum()) == len(pos) * m * m          # P7
     rec.close()
+
+
+@pytest.mark.parametrize("case", ["fig3-small", "random-wrap", "corner"])
+def test_periodic_tile_lists_and_cover_counts_bit_exact(lib, oracle, case):
+    """sharp_plan_periodic (reading G25): lists and counts against the oracle's brute force over wrapped
+    pixels, on shapes that are not multiples of the tile edge."""
+    if case == "fig3-small":
+        cfg = synth.reduced(synth.config(6), 17); pos, shape, m = synth.positions(cfg), cfg.shape, cfg.m     # 170 x 170
+    elif case == "random-wrap":
+        rng = np.random.default_rng(6)
+        m, shape = 64, (131, 97)                           # 97 - 64 = 33 >= TILE - 1
+        pos = np.stack([rng.integers(0, shape[0], 41), rng.integers(0, shape[1], 41)], 1).astype(np.int32)
+    else:
+        m, shape = 64, (95, 200)                           # the smallest legal margin on rows: 95 - 64 = 31
+        pos = np.array([[94, 199], [0, 0], [31, 136], [32, 137], [63, 1]], np.int32)
+    rec = sharp.Reconstruction(m, pos, shape, device=None, periodic=True)
+    ptr, frames = rec.tile_lists()
+    optr, oframes = oracle.tile_lists_periodic(m, pos, shape, sharp.TILE)
+    assert np.array_equal(ptr, optr) and np.array_equal(frames, oframes)
+    cnt = rec.cover_counts()
+    assert np.array_equal(cnt, oracle.cover_counts(m, pos, shape)) and int(cnt.sum()) == len(pos) * m * m
+    rec.close()
+
+
+def test_periodic_plan_validation(lib):
+    def plan(m, pos, shape):
+        pos = np.ascontiguousarray(pos, dtype=np.int32)
+        h = C.c_void_p(None)
+        rc = lib.sharp_plan_periodic(C.byref(h), m, len(pos), pos.ctypes.data_as(C.c_void_p), shape[0], shape[1])
+        if rc == sharp.SHARP_OK:
+            lib.sharp_destroy(h)
+        return rc
+    assert plan(64, [[99, 99]], (100, 100)) == sharp.SHARP_OK          # anywhere in the image
+    assert plan(64, [[100, 0]], (100, 100)) == sharp.SHARP_EINVAL       # but inside it
+    assert plan(64, [[0, 0]], (94, 100)) == sharp.SHARP_EINVAL          # margin 30 < TILE - 1
+    assert plan(64, [[0, 0]], (95, 95)) == sharp.SHARP_OK
