@@ -51,12 +51,16 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[n-1]; 2 = medium raster (default)")
+    ap.add_argument("--config", type=int, default=2,
+                    help="BASELINE.json configs[n-1]; 2 = medium raster (default); 6 = the paper's Fig. 3 shape (periodic)")
     ap.add_argument("--iters", type=int, default=0, help="RAAR iterations per step (0 = the config's own count)")
     ap.add_argument("--grid", type=int, default=0, help="reduce the raster to grid x grid (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the config-4 (m = 256) block of the default run")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE scan, its frames partitioned over the ranks by region, object numerator all-reduced "
+                         "every iteration (sharp_set_sharded; strong scaling) instead of one independent scan per rank")
     return ap.parse_args()
 
 
@@ -75,7 +79,8 @@ def workload(args, rank=0):
 def workload_name(cfg, iters):
     return (f"{cfg.name}: {cfg.K} frames {cfg.m}x{cfg.m} c64, object {cfg.shape[0]}x{cfg.shape[1]}, "
             f"beta {cfg.beta}, {iters} RAAR iterations/step, probe "
-            + (f"refined every {cfg.refine_every}" if cfg.refine_every else "fixed"))
+            + (f"refined every {cfg.refine_every}" if cfg.refine_every else "fixed")
+            + (", periodic boundary" if cfg.periodic else ""))
 
 
 # ---- the CPU oracle, timed as it stands (cpu_baseline and --impl reference) ---------------------------------------
@@ -84,6 +89,8 @@ def oracle_sample(args):
     import synth
     cfg = synth.config(args.config)
     g = {64: 10, 128: 12, 256: 6, 512: 9}[cfg.m]          # frames: 100 / 144 / 36 / 9
+    if cfg.periodic:
+        g = 16                                              # the torus must stay larger than the frame: 160 x 160
     scfg = synth.reduced(cfg, min(g, cfg.grid))
     its = 2 if cfg.m <= 128 else 1
     return scfg, its
@@ -223,14 +230,22 @@ def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e
     cfg = synth.config(config_number)
     if args.grid:
         cfg = synth.reduced(cfg, args.grid)
-    if rank:
+    sharded = bool(args.sharded) and world > 1
+    if rank and not sharded:
         cfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
     iters = args.iters or cfg.iters
     pos, shape, I, w0, obj, wt = synth.make(cfg)
-    K, m = cfg.K, cfg.m
+    K_total = cfg.K
+    if sharded:                                  # this rank's region of the one scan
+        from paper_1602_01448_b200.sharding import partition_by_region
+        mine = partition_by_region(pos, world)[rank]
+        pos, I = pos[mine], np.ascontiguousarray(I[mine])
+    K, m = len(pos), cfg.m
     I_host = torch.from_numpy(np.ascontiguousarray(I)).pin_memory()
     w_host = torch.from_numpy(np.ascontiguousarray(w0)).pin_memory()
-    rec = sharp.Reconstruction(m, pos, shape, device=dev)
+    rec = sharp.Reconstruction(m, pos, shape, device=dev, periodic=bool(cfg.periodic))
+    if sharded:
+        rec.set_sharded(lambda t: dist.all_reduce(t), K_total)
     rec.set_probe_refine(cfg.refine_every)
     I_dev = I_host.to(dev)
     rec.set_intensities(I_dev)
@@ -267,7 +282,7 @@ def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e
     launches = rec.launch_count() - l0
     clocks = sampler.stop() if sampler else None
     ms = max_over_ranks(ms, dist, dev)
-    value = job_value(world, K, iters, steps, ms)
+    value = job_value(1 if sharded else world, K_total, iters, steps, ms)
 
     # ---- second pass over the same steps with events around every launch: per-kernel durations -----------------
     rec.profile(True)
@@ -318,7 +333,7 @@ def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e
         torch.cuda.synchronize(dev)
         dt = time.perf_counter() - t0
         dt = max_over_ranks(dt, dist, dev)
-        e2e = {"value": world * K * iters * n_e2e / dt, "unit": UNIT,
+        e2e = {"value": (1 if sharded else world) * K_total * iters * n_e2e / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(I_host.numel() * 4 + w_host.numel() * 8),
                "d2h_bytes_per_step": int(shape[0] * shape[1] * 8 + m * m * 8 + 12),
                "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
@@ -326,7 +341,7 @@ def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e
     eps0 = None
     if hasattr(rec, "eps0"):
         try:
-            eps0 = float(rec.eps0(obj))      # Eq. 14: error against the known synthetic object (the last step's result)
+            eps0 = float(rec.eps0(obj, wt))  # Eq. 14: error against the known synthetic object and its illumination
         except Exception:
             eps0 = None
     rec.close()
@@ -335,7 +350,7 @@ def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e
     return {
         "value": value, "ms": ms, "steps": steps, "iters": iters, "eps": [float(x) for x in eps], "eps0": eps0,
         "launches": int(launches), "clocks": clocks, "roofline": roofline, "e2e": e2e,
-        "workload": workload_name(cfg, iters), "K": K, "m": m,
+        "workload": workload_name(cfg, iters), "K": K, "m": m, "sharded": sharded,
         "l2": "inputs larger than L2 (frame state 2x%.0f MB + amplitudes %.0f MB per iteration vs 126 MB L2)"
               % (K * m * m * 8 / 1e6, K * m * m * 4 / 1e6),
     }
@@ -380,7 +395,8 @@ def run_ours(args):
     def block(r, config_number):
         return {
             "config": {"workload": r["workload"], "config_number": config_number, "l2": r["l2"],
-                       "parallelism": "independent scan per GPU, no collective" if world > 1 else "single GPU",
+                       "parallelism": ("one scan sharded by region over the GPUs, object numerator all-reduced every iteration"
+                                       if r["sharded"] else "independent scan per GPU, no collective") if world > 1 else "single GPU",
                        "step": "set_object(flat) + iterate(iters, beta) + errors()"},
             "value": r["value"], "unit": UNIT, "steps": r["steps"], "ms_per_step": r["ms"] / r["steps"],
             "ms_per_iteration": r["ms"] / r["steps"] / r["iters"], "eps": r["eps"], "eps0": r["eps0"],
@@ -390,8 +406,8 @@ def run_ours(args):
     m1 = block(main_, args.config)
     line = {
         "metric": METRIC, "value": m1["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": warm, "ms_per_step": m1["ms_per_step"], "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": m1["config"],
+        "warmup": warm, "ms_per_step": m1["ms_per_step"], "higher_is_better": True,
+        "scaling": "strong" if main_["sharded"] else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": m1["config"],
         "ms_per_iteration": m1["ms_per_iteration"], "eps": m1["eps"], "eps0": m1["eps0"],
         "gpu_launches": m1["gpu_launches"] + (second["launches"] if second else 0),
         "clocks": m1["clocks"], "roofline": m1["roofline"], "e2e": m1["e2e"], "cpu_baseline": cpu,

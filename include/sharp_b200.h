@@ -178,6 +178,24 @@ int sharp_init_probe(sharp_plan_t *p);
 int sharp_init_object_random(sharp_plan_t *p, unsigned long long seed);
 int sharp_op_random_object(sharp_plan_t *p, unsigned long long seed, float *out_dev);
 
+/* ---- sharded reconstruction (Fig. 2) --------------------------
+ * "Summing the frames onto an image (Q*z) requires a reduction for every image pixel across neighboring MPI nodes ...
+ * the resulting image is summed across all MPI nodes."  One process per GPU; every rank makes a plan with ITS frames
+ * (positions and intensities of its part of the scan, by region or any other partition) and the FULL object size.
+ * sharp_set_sharded gives the plan the collective: fn(user, dev_ptr, count, is_double) must replace the `count`
+ * float32 (is_double = 0) or float64 (is_double = 1) values at DEVICE pointer dev_ptr (inside the plan's workspace) by
+ * their SUM over all ranks, ordered after the work already enqueued on the plan's stream and before anything enqueued
+ * on it later (e.g. an NCCL all-reduce on that stream), and return 0; anything else fails the calling sharp_* call
+ * with SHARP_ECUDA.  The library calls it wherever the method sums over frames: Q*Q and ||a||^2 when the inputs are
+ * set, the object numerator once per iteration (8 bytes per object pixel), the Eq. 10 sums (12 m^2 bytes) per
+ * illumination update, three doubles per sharp_errors, m^2 doubles in sharp_init_probe.  All ranks must make the same
+ * sequence of calls.  K_total = number of frames of the whole scan (a_rms of reading G4 is global).  Must be called
+ * before sharp_set_intensities / sharp_set_probe; fn = NULL returns to the single-GPU plan.
+ * With the numerator summed in rank order instead of ascending frame index the result differs from the single-GPU
+ * run by rounding only (parity <= 1e-5 against the oracle either way). */
+typedef int (*sharp_allreduce_fn)(void *user, void *dev_ptr, size_t count, int is_double);
+int sharp_set_sharded(sharp_plan_t *p, sharp_allreduce_fn fn, void *user, long long K_total);
+
 /* ---- illumination constraints and re-centring (step 7) -------
  * Applied after every illumination update of Eq. 10 inside sharp_iterate, in the paper's order:
  *   kind 1 (mask)       w <- F^{-1}{ (F w) m_w }

@@ -56,6 +56,7 @@ _SIGNATURES = {
     "sharp_init_probe": (_i, [_vp]),
     "sharp_init_object_random": (_i, [_vp, C.c_ulonglong]),
     "sharp_op_random_object": (_i, [_vp, C.c_ulonglong, _vp]),
+    "sharp_set_sharded": (_i, [_vp, _vp, _vp, _ll]),
     "sharp_set_probe_constraint": (_i, [_vp, _i, _vp]),
     "sharp_set_probe_recentre": (_i, [_vp, _i]),
     "sharp_get_probe_shift": (_i, [_vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]),
@@ -313,6 +314,15 @@ class Reconstruction:
         out = self._new(self.shape, self._torch.complex64)
         self._check(self.lib.sharp_op_random_object(self._plan, C.c_ulonglong(int(seed)), _ptr(out)))
         return out
+
+    def set_sharded(self, allreduce, K_total):
+        """This plan holds one rank's frames of a scan of K_total frames; allreduce(t) sums the torch tensor t in place
+        over all ranks on the current stream (e.g. lambda t: torch.distributed.all_reduce(t)).  Call before
+        set_intensities / set_probe."""
+        from .sharding import make_allreduce_callback
+        self._ar_fn = make_allreduce_callback(self._ws, allreduce, self._stream) if allreduce is not None else None
+        fn = C.cast(self._ar_fn, _vp) if self._ar_fn is not None else _vp(None)
+        self._check(self.lib.sharp_set_sharded(self._plan, fn, None, int(K_total)))
 
     def set_probe_constraint(self, kind, con=None):
         kind = {"none": 0, "mask": 1, "amplitude": 2}.get(kind, kind)

@@ -141,6 +141,12 @@ __global__ void k_scalars(int nparts, const double *partials, int K, double tau,
     }
 }
 
+// sharded plan: A2 has been summed over the ranks; thr2 follows from the global mean (K_total frames)
+__global__ void k_scalars_thr(long long K_total, double tau, DevScalars *sc)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) sc->thr2 = (float)(tau * tau * sc->A2 / (double)K_total);
+}
+
 // sums gridDim-many triples in index order into out[3] (eps numerators, doubles)
 __global__ void k_sum_triples(int n, const double *partials, double *out)
 {
@@ -184,10 +190,51 @@ struct OverlapArgs {
     float2 *psi_z;          // ITER in/out, REGATHER out
     const float2 *psi_v_in; // REGATHER
     float2 *psi_v_out;      // ITER
+    float2 *num_out;        // not NULL: write the raw numerator here and skip the epilogue (sharded plan)
     float beta;
 };
 
+// Object-space epilogue of one pixel p with numerator num(p) (written once; the gather kernel and the sharded
+// two-step path both end here):
+//   OV_L         out[p] = num/den, 0 where den == 0 (reading G5)
+//   OV_ITER      psi_c = num/den; psi_y = (psi_c - beta psi_z)/(1 - 2 beta); psi_v[p] = beta (2 psi_y - psi_z); psi_z[p] = psi_y
+//   OV_REGATHER  psi_z[p] = (num + psi_v[p] cross[p])/den
 template <int MODE>
+__device__ __forceinline__ void object_epilogue(const OverlapArgs &A, size_t p, float2 num)
+{
+    const float d = A.den[p];
+    const bool lit = d > 0.f;
+    if constexpr (MODE == OV_L) {
+        A.out[p] = lit ? make_float2(num.x / d, num.y / d) : make_float2(0.f, 0.f);
+    } else if constexpr (MODE == OV_ITER) {
+        float2 py = make_float2(0.f, 0.f), pv = py;
+        if (lit) {
+            const float2 pz = A.psi_z[p];
+            const float inv = 1.0f / (1.0f - 2.0f * A.beta);
+            py.x = (num.x / d - A.beta * pz.x) * inv;
+            py.y = (num.y / d - A.beta * pz.y) * inv;
+            pv.x = A.beta * (2.0f * py.x - pz.x);
+            pv.y = A.beta * (2.0f * py.y - pz.y);
+        }
+        A.psi_z[p] = py;
+        A.psi_v_out[p] = pv;
+    } else {  // OV_REGATHER
+        float2 o = make_float2(0.f, 0.f);
+        if (lit) {
+            float2 t = num;
+            if (A.psi_v_in != nullptr) t = cadd(t, cmul(A.psi_v_in[p], A.cross[p]));
+            o = make_float2(t.x / d, t.y / d);
+        }
+        A.psi_z[p] = o;
+    }
+}
+
+// The gather loop.  M is a template parameter so that the four rows of a thread are immediate offsets from one pointer
+// per array.  The tile's list is staged in shared memory in chunks of CH entries as, per frame: the element offset of
+// the tile's corner pixel inside the frame data and inside the probe (so a thread's address is that plus its own
+// constant ty M + tx), and the range of tile rows / columns the frame covers, packed in one word.  UNR frames are in
+// flight per thread at a time and are accumulated in list order (ascending frame index: reading G17).
+template <int M, int MODE>
 __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
 {
     const int tile = blockIdx.x;
@@ -195,8 +242,8 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int pc = tc * TILE + tx;
     const int pr0 = tr * TILE + ty;
-    const int m = A.m;
     const int beg = A.tile_ptr[tile], end = A.tile_ptr[tile + 1];
+    const int toff = ty * M + tx;
 
     float2 num[4], cr[4];
     float dn[4];
@@ -207,11 +254,10 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
         dn[k] = 0.f;
     }
 
-    // The tile's list (frame index and position) is staged in shared memory in chunks, so the loads of the frame
-    // data do not hang off a chain of dependent index loads; UNR frames are in flight per thread at a time and
-    // are accumulated in list order (ascending frame index: reading G17).
     constexpr int CH = 128, UNR = 4;
-    __shared__ int s_fi[CH], s_xr[CH], s_xc[CH];
+    __shared__ long long s_foff[CH];     // fi M^2 + (tile row0 - x_r) M + (tile col0 - x_c): may be negative before toff is added
+    __shared__ int s_woff[CH];           // the same without the frame term
+    __shared__ unsigned s_rng[CH];       // r_lo | r_hi << 8 | c_lo << 16 | c_hi << 24  (tile-local, half-open)
     for (int base = beg; base < end; base += CH) {
         const int n = min(CH, end - base);
         __syncthreads();
@@ -224,9 +270,12 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
                 if (xr > tr * TILE + TILE - 1) xr -= A.nr;
                 if (xc > tc * TILE + TILE - 1) xc -= A.nc;
             }
-            s_fi[j] = fi;
-            s_xr[j] = xr;
-            s_xc[j] = xc;
+            const int dr = tr * TILE - xr, dc = tc * TILE - xc;          // frame coordinates of the tile's corner
+            const int wo = dr * M + dc;
+            s_woff[j] = wo;
+            s_foff[j] = (long long)fi * (M * M) + wo;
+            const int rlo = max(0, -dr), rhi = min(TILE, M - dr), clo = max(0, -dc), chi = min(TILE, M - dc);
+            s_rng[j] = (unsigned)rlo | ((unsigned)rhi << 8) | ((unsigned)clo << 16) | ((unsigned)chi << 24);
         }
         __syncthreads();
         for (int e0 = 0; e0 < n; e0 += UNR) {
@@ -235,21 +284,23 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
 #pragma unroll
             for (int u = 0; u < UNR; ++u) {
                 const int e = min(e0 + u, n - 1);
-                const int cc = pc - s_xc[e];
-                const bool colok = (e0 + u < n) && ((unsigned)cc < (unsigned)m);
-                const float2 *fb = (MODE == OV_DEN) ? nullptr : A.f + (size_t)s_fi[e] * m * m;
+                const unsigned rng = s_rng[e];
+                const int rlo = rng & 255, rh = ((rng >> 8) & 255) - rlo, clo = (rng >> 16) & 255, cw = (rng >> 24) - clo;
+                const bool colok = (e0 + u < n) && ((unsigned)(tx - clo) < (unsigned)cw);
+                const int wo = s_woff[e] + toff;
+                const float2 *wp = A.w_a + wo;
+                const float2 *fp = (MODE == OV_DEN) ? nullptr : A.f + (s_foff[e] + toff);
+                const float2 *bp = (MODE == OV_DEN && A.w_b != nullptr) ? A.w_b + wo : nullptr;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    const int rr = pr0 + 8 * k - s_xr[e];
-                    ok[u][k] = colok && ((unsigned)rr < (unsigned)m);
-                    const int off = rr * m + cc;
+                    ok[u][k] = colok && ((unsigned)(ty + 8 * k - rlo) < (unsigned)rh);
                     wa[u][k] = make_float2(0.f, 0.f);
                     fv[u][k] = make_float2(0.f, 0.f);
                     wb[u][k] = make_float2(0.f, 0.f);
                     if (ok[u][k]) {
-                        wa[u][k] = __ldg(A.w_a + off);
-                        if constexpr (MODE != OV_DEN) fv[u][k] = __ldcs(fb + off);
-                        if constexpr (MODE == OV_DEN) { if (A.w_b != nullptr) wb[u][k] = __ldg(A.w_b + off); }
+                        wa[u][k] = __ldg(wp + 8 * k * M);
+                        if constexpr (MODE != OV_DEN) fv[u][k] = __ldcs(fp + 8 * k * M);
+                        if constexpr (MODE == OV_DEN) { if (bp != nullptr) wb[u][k] = __ldg(bp + 8 * k * M); }
                     }
                 }
             }
@@ -284,33 +335,20 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
             A.den[p] = dn[k];
             if (A.w_b != nullptr) A.cross[p] = cr[k];
         } else {
-            const float d = A.den[p];
-            const bool lit = d > 0.f;
-            if constexpr (MODE == OV_L) {
-                A.out[p] = lit ? make_float2(num[k].x / d, num[k].y / d) : make_float2(0.f, 0.f);
-            } else if constexpr (MODE == OV_ITER) {
-                float2 py = make_float2(0.f, 0.f), pv = py;
-                if (lit) {
-                    const float2 pz = A.psi_z[p];
-                    const float inv = 1.0f / (1.0f - 2.0f * A.beta);
-                    py.x = (num[k].x / d - A.beta * pz.x) * inv;
-                    py.y = (num[k].y / d - A.beta * pz.y) * inv;
-                    pv.x = A.beta * (2.0f * py.x - pz.x);
-                    pv.y = A.beta * (2.0f * py.y - pz.y);
-                }
-                A.psi_z[p] = py;
-                A.psi_v_out[p] = pv;
-            } else {  // OV_REGATHER
-                float2 o = make_float2(0.f, 0.f);
-                if (lit) {
-                    float2 t = num[k];
-                    if (A.psi_v_in != nullptr) t = cadd(t, cmul(A.psi_v_in[p], A.cross[p]));
-                    o = make_float2(t.x / d, t.y / d);
-                }
-                A.psi_z[p] = o;
-            }
+            if (A.num_out != nullptr) A.num_out[p] = num[k];     // sharded plan: the sum over ranks comes first
+            else object_epilogue<MODE>(A, p, num[k]);
         }
     }
+}
+
+// The object-space epilogue alone, on a numerator that was summed over the ranks of a sharded reconstruction
+// ("the resulting image is summed across all MPI nodes").
+template <int MODE>
+__global__ void __launch_bounds__(256) k_object_epilogue(OverlapArgs A, const float2 *num)
+{
+    const size_t n = (size_t)A.nr * A.nc;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (size_t)gridDim.x * blockDim.x)
+        object_epilogue<MODE>(A, p, num[p]);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -343,8 +381,10 @@ __global__ void __launch_bounds__(256) k_probe_partial(int m, int K, int chunk, 
     pden[(size_t)blockIdx.y * m * m + pix] = den;
 }
 
+// raw != NULL (sharded plan): the sums (num.x, num.y, den) go to raw[3 pix ..] for the sum over ranks and
+// k_probe_divide finishes
 __global__ void __launch_bounds__(256) k_probe_final(int m, int nchunks, const float2 *pnum, const float *pden,
-                                                      const float2 *w_old, float2 *w_new)
+                                                      const float2 *w_old, float2 *w_new, float *raw)
 {
     const int pix = blockIdx.x * blockDim.x + threadIdx.x;
     float2 num = make_float2(0.f, 0.f);
@@ -355,7 +395,20 @@ __global__ void __launch_bounds__(256) k_probe_final(int m, int nchunks, const f
         num.y += a.y;
         den += pden[(size_t)j * m * m + pix];
     }
+    if (raw != nullptr) {
+        raw[3 * pix + 0] = num.x;
+        raw[3 * pix + 1] = num.y;
+        raw[3 * pix + 2] = den;
+        return;
+    }
     w_new[pix] = den > 0.f ? make_float2(num.x / den, num.y / den) : w_old[pix];
+}
+
+__global__ void __launch_bounds__(256) k_probe_divide(const float *raw, const float2 *w_old, float2 *w_new)
+{
+    const int pix = blockIdx.x * blockDim.x + threadIdx.x;
+    const float den = raw[3 * pix + 2];
+    w_new[pix] = den > 0.f ? make_float2(raw[3 * pix] / den, raw[3 * pix + 1] / den) : w_old[pix];
 }
 
 __global__ void k_fill_c64(size_t n, float2 *p, float2 v)

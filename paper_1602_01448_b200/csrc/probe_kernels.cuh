@@ -87,15 +87,24 @@ __global__ void __launch_bounds__(256) k_mean_frame_partial(int m, int K, int ch
     part[(size_t)blockIdx.y * mm + slot] = s;
 }
 
-__global__ void __launch_bounds__(256) k_mean_frame_final(int m, int K, int nchunks, const double *part, float2 *abar)
+// chunks -> part[0 .. m*m) in ascending chunk order (each thread reads and then writes only its own slot)
+__global__ void __launch_bounds__(256) k_mean_frame_sum(int m, int nchunks, double *part)
 {
     const int slot = blockIdx.x * blockDim.x + threadIdx.x;
     const size_t mm = (size_t)m * m;
     double s = 0.0;
     for (int j = 0; j < nchunks; ++j) s += part[(size_t)j * mm + slot];
+    part[slot] = s;
+}
+
+// K = the frames of the WHOLE scan (a sharded plan sums part[] over its ranks first)
+__global__ void __launch_bounds__(256) k_mean_frame_sqrt(int m, long long K, const double *part, float2 *abar)
+{
+    const int slot = blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t mm = (size_t)m * m;
     int u, v;
     amp_slot_freq(m, slot, u, v);
-    abar[(size_t)u * m + v] = make_float2((float)sqrt(s * (double)mm / (double)K), 0.f);
+    abar[(size_t)u * m + v] = make_float2((float)sqrt(part[slot] * (double)mm / (double)K), 0.f);
 }
 
 // out[(r + d_r) mod m][(c + d_c) mod m] = in[r][c];  the shift is read from device memory (written by k_probe_moments)

@@ -57,7 +57,7 @@ struct sharp_plan_s {
     // workspace offsets
     size_t o_a = 0, o_c[2] = {0, 0}, o_psi_z = 0, o_psi_v[2] = {0, 0}, o_den = 0, o_cross = 0, o_w[4] = {0, 0, 0, 0}, o_scratch = 0,
            o_pos = 0, o_tile_ptr = 0, o_tile_frames = 0, o_partials = 0, o_err_partials = 0, o_err_sums = 0, o_pnum = 0,
-           o_pden = 0, o_scalars = 0, o_wtmp[3] = {0, 0, 0}, o_wcon = 0, o_pscal = 0, o_quads = 0, o_quad_sum = 0, o_total = 0;
+           o_pden = 0, o_scalars = 0, o_wtmp[3] = {0, 0, 0}, o_wcon = 0, o_pscal = 0, o_quads = 0, o_quad_sum = 0, o_num = 0, o_praw = 0, o_total = 0;
 
     // state
     bool have_I = false, have_probe = false, have_frames = false, have_prev = false;
@@ -66,6 +66,11 @@ struct sharp_plan_s {
     bool prev_psi_v_zero = true;
     int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
     int refine_every = 0;
+    // sharded reconstruction: this plan holds a subset of the frames; every sum over frames is
+    // completed by the caller's all-reduce before it is used
+    sharp_allreduce_fn allreduce = nullptr;
+    void *ar_user = nullptr;
+    long long K_total = 0;
     int probe_constraint = 0;          // 0 none, 1 Fourier mask m_w, 2 Fourier amplitude a_w
     bool probe_recentre = false;       // centre-of-mass shift after every illumination update
     long long it = 0;
@@ -268,12 +273,43 @@ OverlapArgs base_overlap_args(sharp_plan_t *p)
     return a;
 }
 
-template <int MODE>
-int overlap_launch(sharp_plan_t *p, const OverlapArgs &a)
+// sum over the ranks of a sharded plan, in place, ordered after the work already enqueued on the plan's stream (the
+// caller's function enqueues its collective on that stream); no-op for an ordinary plan
+int reduce_over_ranks(sharp_plan_t *p, void *dev_ptr, size_t count, bool is_double)
 {
-    ProfScope prof(p, MODE == OV_ITER ? SHARP_PROF_OVERLAP : SHARP_PROF_OTHER);
-    k_overlap<MODE><<<p->tiles_r * p->tiles_c, 256, 0, p->stream>>>(a);
+    if (!p->allreduce) return SHARP_OK;
+    if (p->allreduce(p->ar_user, dev_ptr, count, is_double ? 1 : 0) != 0)
+        return fail(p, SHARP_ECUDA, "the all-reduce callback of the sharded plan failed");
+    return SHARP_OK;
+}
+
+template <int MODE>
+int overlap_launch(sharp_plan_t *p, const OverlapArgs &a_in)
+{
+    OverlapArgs a = a_in;
+    const bool two_step = p->allreduce != nullptr && MODE != OV_DEN;
+    if (two_step) a.num_out = p->dp<float2>(p->o_num);
+    {
+        ProfScope prof(p, MODE == OV_ITER ? SHARP_PROF_OVERLAP : SHARP_PROF_OTHER);
+        const int grid = p->tiles_r * p->tiles_c;
+        switch (p->m) {
+        case 64: k_overlap<64, MODE><<<grid, 256, 0, p->stream>>>(a); break;
+        case 128: k_overlap<128, MODE><<<grid, 256, 0, p->stream>>>(a); break;
+        case 256: k_overlap<256, MODE><<<grid, 256, 0, p->stream>>>(a); break;
+        default: k_overlap<512, MODE><<<grid, 256, 0, p->stream>>>(a); break;
+        }
+    }
     CK_LAUNCH("k_overlap");
+    if (MODE == OV_DEN) {
+        if (int rc = reduce_over_ranks(p, a.den, p->nobj(), false)) return rc;
+        if (a.w_b != nullptr)
+            if (int rc = reduce_over_ranks(p, a.cross, 2 * p->nobj(), false)) return rc;
+    } else if (two_step) {
+        if (int rc = reduce_over_ranks(p, a.num_out, 2 * p->nobj(), false)) return rc;
+        ProfScope prof(p, SHARP_PROF_OTHER);
+        k_object_epilogue<MODE><<<grid_for(p->nobj()), 256, 0, p->stream>>>(a, a.num_out);
+        CK_LAUNCH("k_object_epilogue");
+    }
     return SHARP_OK;
 }
 
@@ -476,6 +512,8 @@ static int make_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, in
     p->o_pscal = take(sizeof(ProbeScalars));
     p->o_quads = take((size_t)kQuadBlocks * 4 * 8);
     p->o_quad_sum = take(4 * 8);
+    p->o_num = take(p->nobj() * 8);            // raw object numerator of a sharded plan (summed over ranks in place)
+    p->o_praw = take((size_t)m * m * 3 * 4);   // raw Eq. 10 sums (num.x, num.y, den) of a sharded plan
     p->o_total = o;
     *out = p;
     return SHARP_OK;
@@ -560,6 +598,12 @@ int sharp_set_intensities(sharp_plan_t *p, const float *I_dev)
     CK_LAUNCH("k_amplitudes");
     k_scalars<<<1, 32, 0, p->stream>>>(p->amp_blocks, p->dp<double>(p->o_partials), p->K, kTau, p->dp<DevScalars>(p->o_scalars));
     CK_LAUNCH("k_scalars");
+    if (p->allreduce) {
+        // ||a||^2 and a_rms are those of the whole scan (PAPER.md:196-206 normalise by the global ||a||; reading G4)
+        if (int rc = reduce_over_ranks(p, &p->dp<DevScalars>(p->o_scalars)->A2, 1, true)) return rc;
+        k_scalars_thr<<<1, 32, 0, p->stream>>>(p->K_total, kTau, p->dp<DevScalars>(p->o_scalars));
+        CK_LAUNCH("k_scalars_thr");
+    }
     p->have_I = true;
     return SHARP_OK;
 }
@@ -671,9 +715,15 @@ int sharp_iterate(sharp_plan_t *p, int n, float beta)
             if (slot < 0) return fail(p, SHARP_ECUDA, "internal: no free probe slot");
             const bool post = p->probe_constraint != 0 || p->probe_recentre;
             float2 *w_eq10 = post ? p->dp<float2>(p->o_wtmp[0]) : p->dp<float2>(p->o_w[slot]);
+            float *raw = p->allreduce ? p->dp<float>(p->o_praw) : nullptr;
             k_probe_final<<<mm_i / 256, 256, 0, p->stream>>>(p->m, p->probe_nchunks, p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden),
-                                                             p->dp<float2>(p->o_w[p->w_cur]), w_eq10);
+                                                             p->dp<float2>(p->o_w[p->w_cur]), w_eq10, raw);
             CK_LAUNCH("k_probe_final");
+            if (raw) {
+                if (int rc = reduce_over_ranks(p, raw, (size_t)3 * mm_i, false)) return rc;
+                k_probe_divide<<<mm_i / 256, 256, 0, p->stream>>>(raw, p->dp<float2>(p->o_w[p->w_cur]), w_eq10);
+                CK_LAUNCH("k_probe_divide");
+            }
             if (post)
                 if (int rc = constrain_probe(p, w_eq10, p->dp<float2>(p->o_w[slot]))) return rc;
             p->w_cur = slot;
@@ -742,6 +792,7 @@ int sharp_errors(sharp_plan_t *p, float out[3])
     if (int rc = frame_dispatch<FRAME_ERR>(p, fa, p->frame_grid)) return rc;
     k_sum_triples<<<1, 32, 0, p->stream>>>(p->frame_grid, p->dp<double>(p->o_err_partials), p->dp<double>(p->o_err_sums));
     CK_LAUNCH("k_sum_triples");
+    if (int rc = reduce_over_ranks(p, p->dp<double>(p->o_err_sums), 3, true)) return rc;
     double sums[3];
     DevScalars sc;
     CK(cudaMemcpyAsync(sums, p->dp<void>(p->o_err_sums), sizeof sums, cudaMemcpyDeviceToHost, p->stream));
@@ -892,7 +943,7 @@ int sharp_op_probe(sharp_plan_t *p, const float *psi_dev, const float *z_dev, fl
                                               reinterpret_cast<const float2 *>(psi_dev), p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden));
     CK_LAUNCH("k_probe_partial");
     k_probe_final<<<mm_i / 256, 256, 0, p->stream>>>(p->m, p->probe_nchunks, p->dp<float2>(p->o_pnum), p->dp<float>(p->o_pden),
-                                                     p->dp<float2>(p->o_w[p->w_cur]), reinterpret_cast<float2 *>(out_dev));
+                                                     p->dp<float2>(p->o_w[p->w_cur]), reinterpret_cast<float2 *>(out_dev), nullptr);
     CK_LAUNCH("k_probe_final");
     return SHARP_OK;
 }
@@ -957,8 +1008,11 @@ int sharp_init_probe(sharp_plan_t *p)
     dim3 g(mm / 256, p->probe_nchunks);
     k_mean_frame_partial<<<g, 256, 0, p->stream>>>(p->m, p->K, p->probe_chunk, p->dp<float>(p->o_a), part);
     CK_LAUNCH("k_mean_frame_partial");
-    k_mean_frame_final<<<mm / 256, 256, 0, p->stream>>>(p->m, p->K, p->probe_nchunks, part, p->dp<float2>(p->o_wtmp[0]));
-    CK_LAUNCH("k_mean_frame_final");
+    k_mean_frame_sum<<<mm / 256, 256, 0, p->stream>>>(p->m, p->probe_nchunks, part);
+    CK_LAUNCH("k_mean_frame_sum");
+    if (int rc = reduce_over_ranks(p, part, (size_t)mm, true)) return rc;
+    k_mean_frame_sqrt<<<mm / 256, 256, 0, p->stream>>>(p->m, p->allreduce ? p->K_total : (long long)p->K, part, p->dp<float2>(p->o_wtmp[0]));
+    CK_LAUNCH("k_mean_frame_sqrt");
     if (int rc = fft_single(p, p->dp<float2>(p->o_wtmp[0]), p->dp<float2>(p->o_wtmp[1]), +1)) return rc;
     k_cyclic_shift<<<mm / 256, 256, 0, p->stream>>>(p->m, p->dp<float2>(p->o_wtmp[1]), nullptr, p->dp<float2>(p->o_wtmp[2]));
     CK_LAUNCH("k_cyclic_shift");
@@ -981,6 +1035,19 @@ int sharp_init_object_random(sharp_plan_t *p, unsigned long long seed)
     float *tmp = p->dp<float>(p->o_psi_v[1]);
     if (int rc = sharp_op_random_object(p, seed, tmp)) return rc;
     return sharp_set_object(p, tmp);
+}
+
+// ---- sharded reconstruction --------------------------------------------------------------------
+int sharp_set_sharded(sharp_plan_t *p, sharp_allreduce_fn fn, void *user, long long K_total)
+{
+    if (!p) return SHARP_EINVAL;
+    if (fn != nullptr && K_total < p->K) return fail(p, SHARP_EINVAL, "K_total %lld is smaller than this rank's %d frames", K_total, p->K);
+    if (p->have_I || p->have_probe)
+        return fail(p, SHARP_ESTATE, "sharp_set_sharded must be called before sharp_set_intensities / sharp_set_probe");
+    p->allreduce = fn;
+    p->ar_user = user;
+    p->K_total = fn ? K_total : 0;
+    return SHARP_OK;
 }
 
 // ---- illumination constraints and re-centring --------------------------------------------------
