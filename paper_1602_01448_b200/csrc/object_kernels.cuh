@@ -234,8 +234,17 @@ __device__ __forceinline__ void object_epilogue(const OverlapArgs &A, size_t p, 
 // the tile's corner pixel inside the frame data and inside the probe (so a thread's address is that plus its own
 // constant ty M + tx), and the range of tile rows / columns the frame covers, packed in one word.  UNR frames are in
 // flight per thread at a time and are accumulated in list order (ascending frame index: reading G17).
+#ifndef SHARP_OV_UNR
+#define SHARP_OV_UNR 4
+#endif
+#ifndef SHARP_OV_MINB
+#define SHARP_OV_MINB 3
+#endif
+// The explicit minimum of resident CTAs matters beyond occupancy: with __launch_bounds__(256) alone ptxas (12.9) allocates
+// 39 registers and interleaves every pair of loads with the arithmetic that consumes it (one frame row in flight per
+// thread); with a minimum given it batches the loads of the UNR frames as written (52 registers at 3 CTAs).
 template <int M, int MODE>
-__global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
+__global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
 {
     const int tile = blockIdx.x;
     const int tr = tile / A.tiles_c, tc = tile % A.tiles_c;
@@ -254,7 +263,7 @@ __global__ void __launch_bounds__(256) k_overlap(OverlapArgs A)
         dn[k] = 0.f;
     }
 
-    constexpr int CH = 128, UNR = 4;
+    constexpr int CH = 128, UNR = SHARP_OV_UNR;
     __shared__ long long s_foff[CH];     // fi M^2 + (tile row0 - x_r) M + (tile col0 - x_c): may be negative before toff is added
     __shared__ int s_woff[CH];           // the same without the frame term
     __shared__ unsigned s_rng[CH];       // r_lo | r_hi << 8 | c_lo << 16 | c_hi << 24  (tile-local, half-open)
