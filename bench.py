@@ -215,7 +215,7 @@ def job_value(world, K, iters, steps, ms):
 # ---- our arm ----------------------------------------------------------------------------------------------------
 def spans_per_step(cfg, iters):
     """kernel launches the library brackets with events in one step (sharp_profile caps the record at 8192)."""
-    per_it = 2 + (4 if cfg.refine_every else 0)
+    per_it = 2 + (2 if cfg.refine_every else 0)      # frame + overlap (+ Eq. 10 partial sums + final)
     return per_it * iters + 8
 
 

@@ -172,8 +172,13 @@ __global__ void k_sum_triples(int n, const double *partials, double *out)
 //   OV_ITER      psi_c = num/den; psi_y = (psi_c - beta psi_z)/(1 - 2 beta); psi_v[p] = beta (2 psi_y - psi_z);
 //                psi_z[p] = psi_y                                (object half of RAAR)
 //   OV_REGATHER  psi_z[p] = (num + psi_v[p] cross[p])/den        (L_{w_a}(c + w_b . T psi_v) after w changed)
+//   OV_BLIND     the iteration that follows an illumination update, in ONE pass: with w_a the new illumination, w_b the
+//                one the frames z = f_prev + w_b . T psi_v_in were formed with, and f the new frame-local state c'':
+//                den = sum |w_a|^2, cross = sum conj(w_a) w_b, n0 = sum conj(w_a) f_prev, n1 = sum conj(w_a) f;
+//                psi_z = (n0 + psi_v_in cross)/den  (= L_{w_a} z, what OV_DEN + OV_REGATHER would have produced), then the
+//                OV_ITER epilogue on n1/den with that psi_z; den[p] is written for later use.
 // ---------------------------------------------------------------------------------------------------------
-enum OverlapMode : int { OV_DEN = 0, OV_L = 1, OV_ITER = 2, OV_REGATHER = 3 };
+enum OverlapMode : int { OV_DEN = 0, OV_L = 1, OV_ITER = 2, OV_REGATHER = 3, OV_BLIND = 4 };
 
 struct OverlapArgs {
     int m, nr, nc, tiles_c;
@@ -182,6 +187,7 @@ struct OverlapArgs {
     const int *tile_ptr;
     const int *tile_frames;
     const float2 *f;        // K m m
+    const float2 *f_prev;   // K m m (OV_BLIND: the state the current frames were formed from)
     const float2 *w_a;      // m m
     const float2 *w_b;      // m m (DEN: second probe of the cross term, may be NULL)
     float2 *cross;          // object-sized (DEN out when w_b given, REGATHER in)
@@ -235,14 +241,15 @@ __device__ __forceinline__ void object_epilogue(const OverlapArgs &A, size_t p, 
 // constant ty M + tx), and the range of tile rows / columns the frame covers, packed in one word.  UNR frames are in
 // flight per thread at a time and are accumulated in list order (ascending frame index: reading G17).
 #ifndef SHARP_OV_UNR
-#define SHARP_OV_UNR 4
+#define SHARP_OV_UNR 6
 #endif
 #ifndef SHARP_OV_MINB
-#define SHARP_OV_MINB 3
+#define SHARP_OV_MINB 2
 #endif
 // The explicit minimum of resident CTAs matters beyond occupancy: with __launch_bounds__(256) alone ptxas (12.9) allocates
 // 39 registers and interleaves every pair of loads with the arithmetic that consumes it (one frame row in flight per
-// thread); with a minimum given it batches the loads of the UNR frames as written (52 registers at 3 CTAs).
+// thread); with a minimum given it batches 12-14 loads as written (56 registers).  Measured at config 2 (us per launch):
+// 131 without; UNR 4 / min 3: 104.6; 4 / 4: 104.8; 8 / 3: 104.4; 6 / 2: 101.1.
 template <int M, int MODE>
 __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
 {
@@ -254,16 +261,17 @@ __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
     const int beg = A.tile_ptr[tile], end = A.tile_ptr[tile + 1];
     const int toff = ty * M + tx;
 
-    float2 num[4], cr[4];
+    float2 num[4], cr[4], n0[4];
     float dn[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         num[k] = make_float2(0.f, 0.f);
         cr[k] = make_float2(0.f, 0.f);
+        n0[k] = make_float2(0.f, 0.f);
         dn[k] = 0.f;
     }
 
-    constexpr int CH = 128, UNR = SHARP_OV_UNR;
+    constexpr int CH = 128, UNR = (MODE == OV_BLIND) ? 2 : SHARP_OV_UNR;
     __shared__ long long s_foff[CH];     // fi M^2 + (tile row0 - x_r) M + (tile col0 - x_c): may be negative before toff is added
     __shared__ int s_woff[CH];           // the same without the frame term
     __shared__ unsigned s_rng[CH];       // r_lo | r_hi << 8 | c_lo << 16 | c_hi << 24  (tile-local, half-open)
@@ -288,7 +296,7 @@ __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
         }
         __syncthreads();
         for (int e0 = 0; e0 < n; e0 += UNR) {
-            float2 fv[UNR][4], wa[UNR][4], wb[UNR][4];
+            float2 fv[UNR][4], wa[UNR][4], wb[UNR][4], fp0[UNR][4];
             bool ok[UNR][4];
 #pragma unroll
             for (int u = 0; u < UNR; ++u) {
@@ -299,17 +307,23 @@ __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
                 const int wo = s_woff[e] + toff;
                 const float2 *wp = A.w_a + wo;
                 const float2 *fp = (MODE == OV_DEN) ? nullptr : A.f + (s_foff[e] + toff);
-                const float2 *bp = (MODE == OV_DEN && A.w_b != nullptr) ? A.w_b + wo : nullptr;
+                const float2 *bp = (MODE == OV_BLIND || (MODE == OV_DEN && A.w_b != nullptr)) ? A.w_b + wo : nullptr;
+                const float2 *qp = (MODE == OV_BLIND) ? A.f_prev + (s_foff[e] + toff) : nullptr;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     ok[u][k] = colok && ((unsigned)(ty + 8 * k - rlo) < (unsigned)rh);
                     wa[u][k] = make_float2(0.f, 0.f);
                     fv[u][k] = make_float2(0.f, 0.f);
                     wb[u][k] = make_float2(0.f, 0.f);
+                    fp0[u][k] = make_float2(0.f, 0.f);
                     if (ok[u][k]) {
                         wa[u][k] = __ldg(wp + 8 * k * M);
                         if constexpr (MODE != OV_DEN) fv[u][k] = __ldcs(fp + 8 * k * M);
                         if constexpr (MODE == OV_DEN) { if (bp != nullptr) wb[u][k] = __ldg(bp + 8 * k * M); }
+                        if constexpr (MODE == OV_BLIND) {
+                            wb[u][k] = __ldg(bp + 8 * k * M);
+                            fp0[u][k] = __ldcs(qp + 8 * k * M);
+                        }
                     }
                 }
             }
@@ -328,6 +342,14 @@ __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
                         const float2 f_ = fv[u][k];
                         num[k].x += w_.x * f_.x + w_.y * f_.y;   // conj(w_a) f
                         num[k].y += w_.x * f_.y - w_.y * f_.x;
+                        if constexpr (MODE == OV_BLIND) {
+                            const float2 b_ = wb[u][k], q_ = fp0[u][k];
+                            dn[k] += w_.x * w_.x + w_.y * w_.y;
+                            cr[k].x += w_.x * b_.x + w_.y * b_.y;
+                            cr[k].y += w_.x * b_.y - w_.y * b_.x;
+                            n0[k].x += w_.x * q_.x + w_.y * q_.y;
+                            n0[k].y += w_.x * q_.y - w_.y * q_.x;
+                        }
                     }
                 }
             }
@@ -343,6 +365,22 @@ __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
         if constexpr (MODE == OV_DEN) {
             A.den[p] = dn[k];
             if (A.w_b != nullptr) A.cross[p] = cr[k];
+        } else if constexpr (MODE == OV_BLIND) {
+            const float d = dn[k];
+            A.den[p] = d;
+            float2 pz = make_float2(0.f, 0.f), py = pz, pv = pz;
+            if (d > 0.f) {
+                float2 t = n0[k];
+                if (A.psi_v_in != nullptr) t = cadd(t, cmul(A.psi_v_in[p], cr[k]));
+                pz = make_float2(t.x / d, t.y / d);                     // L_{w_a} z: the re-gathered estimate
+                const float inv = 1.0f / (1.0f - 2.0f * A.beta);
+                py.x = (num[k].x / d - A.beta * pz.x) * inv;
+                py.y = (num[k].y / d - A.beta * pz.y) * inv;
+                pv.x = A.beta * (2.0f * py.x - pz.x);
+                pv.y = A.beta * (2.0f * py.y - pz.y);
+            }
+            A.psi_z[p] = py;
+            A.psi_v_out[p] = pv;
         } else {
             if (A.num_out != nullptr) A.num_out[p] = num[k];     // sharded plan: the sum over ranks comes first
             else object_epilogue<MODE>(A, p, num[k]);

@@ -62,6 +62,7 @@ struct sharp_plan_s {
     // state
     bool have_I = false, have_probe = false, have_frames = false, have_prev = false;
     int cur = 0, vcur = 0;             // c[cur], psi_v[vcur] are the current factored frames
+    bool obj_stale = false;            // den, cross and psi_z do not reflect w_cur yet (deferred after an illumination update)
     bool psi_v_zero = true;            // psi_v[vcur] is identically 0 (z = c)
     bool prev_psi_v_zero = true;
     int w_cur = 0, w_form = 0, w_prev = 0;  // indices into the four probe buffers
@@ -152,10 +153,16 @@ int grid_for(size_t n, int per_block = 256, int cap = 160 * 16)
 #define SHARP_CS256 8
 #endif
 constexpr int kNT256 = SHARP_NT256;      // threads per CTA (strip of 32 kNT256 values) at m = 256
-constexpr int kCluster256 = SHARP_CS256, kCluster512 = 8;
+#ifndef SHARP_CS512
+#define SHARP_CS512 8
+#endif
+constexpr int kCluster256 = SHARP_CS256, kCluster512 = SHARP_CS512;
 
 // m >= 256: clusters in flight, each owning one scratch frame (m^2 c64) that should stay resident in L2
-int max_scratch_clusters(int m) { return m == 256 ? 80 : 40; }
+#ifndef SHARP_SCR512
+#define SHARP_SCR512 40
+#endif
+int max_scratch_clusters(int m) { return m == 256 ? 80 : SHARP_SCR512; }
 
 int cluster_size(int m) { return m <= 128 ? 1 : (m == 256 ? kCluster256 : kCluster512); }
 
@@ -220,6 +227,10 @@ cudaError_t kernel_prepare(KernelT kern, int nt, int smem, int cs, int sms, int 
 {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
+    if (cs > 8) {      // clusters of 16 are beyond the portable size
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
     if (cs == 1) {
         int bps = 0;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, nt, smem);
@@ -287,10 +298,10 @@ template <int MODE>
 int overlap_launch(sharp_plan_t *p, const OverlapArgs &a_in)
 {
     OverlapArgs a = a_in;
-    const bool two_step = p->allreduce != nullptr && MODE != OV_DEN;
+    const bool two_step = p->allreduce != nullptr && MODE != OV_DEN && MODE != OV_BLIND;
     if (two_step) a.num_out = p->dp<float2>(p->o_num);
     {
-        ProfScope prof(p, MODE == OV_ITER ? SHARP_PROF_OVERLAP : SHARP_PROF_OTHER);
+        ProfScope prof(p, (MODE == OV_ITER || MODE == OV_BLIND) ? SHARP_PROF_OVERLAP : SHARP_PROF_OTHER);
         const int grid = p->tiles_r * p->tiles_c;
         switch (p->m) {
         case 64: k_overlap<64, MODE><<<grid, 256, 0, p->stream>>>(a); break;
@@ -334,6 +345,16 @@ int regather_psi_z(sharp_plan_t *p)
     return overlap_launch<OV_REGATHER>(p, a);
 }
 
+// After an illumination update inside sharp_iterate the new Q*Q, the cross term and the re-gathered psi_z are deferred:
+// the next iteration's overlap produces them in the same pass (OV_BLIND).  Everything else that reads them calls this.
+int ensure_object_state(sharp_plan_t *p)
+{
+    if (!p->obj_stale) return SHARP_OK;
+    p->obj_stale = false;
+    if (int rc = rebuild_den(p)) return rc;
+    return regather_psi_z(p);
+}
+
 // persistent grid of the frame kernels: one CTA (m <= 128) or one cluster (m >= 256) per resident slot, never more
 // than there are frames; sharp_set_frame_slots lowers it (tests force several rounds per CTA that way)
 void update_frame_grid(sharp_plan_t *p)
@@ -365,6 +386,11 @@ int check_ready(sharp_plan_t *p, bool need_I, bool need_probe)
 // frames installed directly in c[cur] (z = c): reset the factored state around them
 int adopt_frames(sharp_plan_t *p)
 {
+    if (p->obj_stale) {                  // the old frames are gone: only Q*Q of the current illumination is still owed
+        p->obj_stale = false;
+        p->have_frames = false;
+        if (int rc = rebuild_den(p)) return rc;
+    }
     p->psi_v_zero = true;
     p->have_prev = false;
     p->w_form = p->w_cur;
@@ -583,6 +609,7 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     CK(cudaStreamSynchronize(p->stream));  // the host vectors may be read until here
     p->bound = true;
     p->have_I = p->have_probe = p->have_frames = p->have_prev = false;
+    p->obj_stale = false;
     p->cur = p->vcur = 0;
     p->w_cur = p->w_form = p->w_prev = 0;
     p->psi_v_zero = p->prev_psi_v_zero = true;
@@ -614,12 +641,14 @@ int sharp_set_probe(sharp_plan_t *p, const float *w_dev)
     if (!w_dev) return fail(p, SHARP_EINVAL, "w_dev is NULL");
     const size_t bytes = (size_t)p->m * p->m * 8;
     if (!p->have_frames) {
+        p->obj_stale = false;
         p->w_cur = p->w_form = p->w_prev = 0;
         CK(cudaMemcpyAsync(p->dp<void>(p->o_w[0]), w_dev, bytes, cudaMemcpyDeviceToDevice, p->stream));
         p->have_probe = true;
         return rebuild_den(p);
     }
     // frames exist: they stay as they are (reading G10); only Q, Q* and Q*Q change from now on
+    p->obj_stale = false;                // whatever was deferred for the replaced illumination is moot
     const int slot = free_probe_slot(p);  // four buffers, three roles: one is always free
     CK(cudaMemcpyAsync(p->dp<void>(p->o_w[slot]), w_dev, bytes, cudaMemcpyDeviceToDevice, p->stream));
     p->w_cur = slot;
@@ -689,7 +718,16 @@ int sharp_iterate(sharp_plan_t *p, int n, float beta)
         oa.psi_z = p->dp<float2>(p->o_psi_z);
         oa.psi_v_out = p->dp<float2>(p->o_psi_v[p->vcur ^ 1]);
         oa.beta = beta;
-        if (int rc = overlap_launch<OV_ITER>(p, oa)) return rc;
+        if (p->obj_stale) {
+            // the illumination changed after the last iteration: Q*Q, the cross term and L_{w_cur} z come out of this pass
+            oa.f_prev = fa.c_in;
+            oa.w_b = p->dp<float2>(p->o_w[p->w_form]);
+            oa.psi_v_in = p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]);
+            p->obj_stale = false;
+            if (int rc = overlap_launch<OV_BLIND>(p, oa)) return rc;
+        } else {
+            if (int rc = overlap_launch<OV_ITER>(p, oa)) return rc;
+        }
         // the new frames are z' = c[cur^1] + w_cur . T psi_v[vcur^1]; the old ones stay readable for eps_Delta
         p->prev_psi_v_zero = p->psi_v_zero;
         p->psi_v_zero = false;
@@ -727,8 +765,12 @@ int sharp_iterate(sharp_plan_t *p, int n, float beta)
             if (post)
                 if (int rc = constrain_probe(p, w_eq10, p->dp<float2>(p->o_w[slot]))) return rc;
             p->w_cur = slot;
-            if (int rc = rebuild_den(p)) return rc;
-            if (int rc = regather_psi_z(p)) return rc;
+            if (p->allreduce) {           // sharded plan: the sums over ranks are taken now
+                if (int rc = rebuild_den(p)) return rc;
+                if (int rc = regather_psi_z(p)) return rc;
+            } else {
+                p->obj_stale = true;      // folded into the next iteration's overlap pass (or taken on demand)
+            }
         }
     }
     return SHARP_OK;
@@ -739,6 +781,7 @@ int sharp_get_object(sharp_plan_t *p, float *out_dev)
     if (int rc = check_ready(p, false, true)) return rc;
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet (call sharp_set_object or sharp_iterate)");
+    if (int rc = ensure_object_state(p)) return rc;
     CK(cudaMemcpyAsync(out_dev, p->dp<void>(p->o_psi_z), p->nobj() * 8, cudaMemcpyDeviceToDevice, p->stream));
     return SHARP_OK;
 }
@@ -777,6 +820,7 @@ int sharp_errors(sharp_plan_t *p, float out[3])
     if (int rc = check_ready(p, true, true)) return rc;
     if (!out) return fail(p, SHARP_EINVAL, "out is NULL");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
+    if (int rc = ensure_object_state(p)) return rc;
     FrameArgs fa = base_frame_args(p);
     fa.c_in = p->dp<float2>(p->o_c[p->cur]);
     fa.psi_v = p->psi_v_zero ? nullptr : p->dp<float2>(p->o_psi_v[p->vcur]);
@@ -900,6 +944,7 @@ int sharp_op_overlap(sharp_plan_t *p, const float *f_dev, float *out_dev)
 {
     if (int rc = check_ready(p, false, true)) return rc;
     if (!f_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
+    if (int rc = ensure_object_state(p)) return rc;
     OverlapArgs a = base_overlap_args(p);
     a.f = reinterpret_cast<const float2 *>(f_dev);
     a.w_a = p->dp<float2>(p->o_w[p->w_cur]);
@@ -978,6 +1023,7 @@ int sharp_eps0(sharp_plan_t *p, const float *psi0_dev, const float *w0_dev, floa
     if (int rc = check_ready(p, false, true)) return rc;
     if (!psi0_dev || !out_host) return fail(p, SHARP_EINVAL, "NULL argument");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
+    if (int rc = ensure_object_state(p)) return rc;
     const float2 *cross = nullptr;
     if (w0_dev != nullptr) {
         // B = Q* Q_{w0} psi_0 = psi_0 . sum_i conj(w) w0: the cross term the Q*Q kernel already knows how to build
