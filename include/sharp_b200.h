@@ -10,8 +10,10 @@
  *
  * Conventions (all calls)
  *   - Arrays are row-major, C-contiguous.  Complex values are interleaved (re, im) float32 ("c64").
- *   - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors); "host" pointers are
- *     ordinary host memory.  Inputs are consumed during the call's stream work; outputs are written into the
+ *   - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors), on the device that owns the
+ *     bound workspace and 16-BYTE ALIGNED (the kernels use 128-bit accesses; a misaligned pointer is SHARP_EINVAL);
+ *     "host" pointers are ordinary host memory.  Calls may be made with any CUDA device current: the library switches
+ *     to the plan's device for the duration of the call.  Inputs are consumed during the call's stream work; outputs are written into the
  *     caller's buffers.  The library never frees caller memory.
  *   - Every call returns 0 (SHARP_OK) or a negative error code; no exception or abort crosses the ABI and a
  *     call that returns SHARP_EINVAL has changed nothing.  sharp_last_error() gives the text.

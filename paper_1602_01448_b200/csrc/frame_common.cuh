@@ -25,6 +25,7 @@ struct FrameArgs {
     const float2 *w_form;    // m m
     const int *pos;          // K x 2
     float2 *scratch;         // gridDim.x * m * m
+    int *sched, *sched_next; // frame counters of the dynamic schedule: this launch's (zero on entry), and the one it zeroes for the next launch
     const DevScalars *sc;
     int K, nr, nc;           // frames, object rows / columns (nr: only the periodic wrap and FRAME_ERR need it)
     float bm;                // beta / m^2

@@ -39,6 +39,16 @@
 #include "fft_regs.cuh"
 #include "frame_common.cuh"
 
+#ifndef SHARP_STAGGER_NS
+#define SHARP_STAGGER_NS 1700
+#endif
+#ifndef SHARP_STAGGER_PHASES
+#define SHARP_STAGGER_PHASES 8
+#endif
+#ifndef SHARP_DYN
+#define SHARP_DYN 1
+#endif
+
 namespace sharp {
 
 template <int M>
@@ -264,26 +274,58 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
     const float bm = A.bm, om = A.om;
     double s_a = 0.0, s_q = 0.0, s_d = 0.0;
 
-    int xr_n = 0, xc_n = 0;      // position of the next frame, fetched one frame ahead
-    if ((int)blockIdx.x < A.K) {
-        xr_n = __ldg(A.pos + 2 * blockIdx.x);
-        xc_n = __ldg(A.pos + 2 * blockIdx.x + 1);
-        if (tid == 0) {
-            prefetch_l2_bulk(A.c_in + (size_t)blockIdx.x * M * M, M * M * 8);
-            if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)blockIdx.x * M * M, M * M * 4);
+    // Frame schedule.  What a CTA needs to know about its next frame (index, position) is CTA-uniform, so it lives in a
+    // double-buffered shared-memory slot instead of registers: thread 0 fills slot (n+1)&1 during frame n (before barrier
+    // 1) and everybody reads it at the top of frame n+1.  The first frame of a CTA is its own index; with SHARP_DYN every
+    // further one comes from a global counter (integer atomicAdd: a CTA that is ahead takes more frames), otherwise it
+    // is the fixed round-robin.  FRAME_ERR always uses the round-robin: its per-CTA partial sums must group the same
+    // frames on every run (bitwise reproducible residuals).
+    constexpr bool DYN = (MODE != FRAME_ERR) && (SHARP_DYN != 0);
+    volatile int *s_sched = reinterpret_cast<volatile int *>(smem_raw + C::E_BYTES + C::TW_BYTES + 16);   // [2][4]
+    if (blockIdx.x == 0 && tid == 0) *A.sched_next = 0;          // the next launch's counter (launches are stream-ordered)
+
+#if SHARP_STAGGER_NS > 0
+    // All CTAs start together, so for the first rounds every SM loads, computes and stores at the same time and the
+    // HBM bursts (47 MB per round at m = 128) are not hidden behind anybody's butterflies: measured 17.3 us per round
+    // in lockstep against 13.5 us once the SMs have drifted apart.  Start the CTAs in SHARP_STAGGER_PHASES phases
+    // instead.  Measured at config 2 (us per launch, dynamic schedule): no stagger 262; 2 x 6800 ns 242.1; 3 x 4500 242.1;
+    // 4 x 3400 243.6; 4 x 4000 245.6; 6 x 2300 242.4; 8 x 1700 242.2; 8 x 2200 245.2.  With the fixed round-robin: 261 / 250.
+    if (MODE == FRAME_ITER && A.K > 2 * (int)gridDim.x) {
+        const unsigned delay = (blockIdx.x % (unsigned)SHARP_STAGGER_PHASES) * (unsigned)SHARP_STAGGER_NS;
+        unsigned long long t0, t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+        do { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); } while (t1 - t0 < delay);
+    }
+#endif
+
+    if (tid == 0) {
+        const int i0 = blockIdx.x;
+        s_sched[0] = i0;
+        if (i0 < A.K) {
+            s_sched[1] = __ldg(A.pos + 2 * i0);
+            s_sched[2] = __ldg(A.pos + 2 * i0 + 1);
+            prefetch_l2_bulk(A.c_in + (size_t)i0 * M * M, M * M * 8);
+            if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)i0 * M * M, M * M * 4);
         }
     }
+    __syncthreads();
 
-    for (int i = blockIdx.x; i < A.K; i += gridDim.x) {
-        const int xr = xr_n, xc = xc_n;
+    for (int par = 0;; par ^= 1) {
+        const int i = s_sched[4 * par];
+        if (i >= A.K) break;
+        const int xr = s_sched[4 * par + 1], xc = s_sched[4 * par + 2];
         const size_t fbase = (size_t)i * M * M;
-        const bool more = i + (int)gridDim.x < A.K;
-        if (more) {
-            xr_n = __ldg(A.pos + 2 * (i + gridDim.x));
-            xc_n = __ldg(A.pos + 2 * (i + gridDim.x) + 1);
-            if (tid == 0) {
-                prefetch_l2_bulk(A.c_in + (size_t)(i + gridDim.x) * M * M, M * M * 8);
-                if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)(i + gridDim.x) * M * M, M * M * 4);
+        // thread 0 asks for the next frame now and consumes the answers just before barrier 1, when this frame's own
+        // loads have long been issued
+        int i_next = i + (int)gridDim.x, ticket = 0, nxr = 0, nxc = 0;
+        if (tid == 0) {
+            if (DYN) {
+                ticket = atomicAdd(A.sched, 1);
+            } else if (i_next < A.K) {
+                nxr = __ldg(A.pos + 2 * i_next);
+                nxc = __ldg(A.pos + 2 * i_next + 1);
+                prefetch_l2_bulk(A.c_in + (size_t)i_next * M * M, M * M * 8);
+                if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)i_next * M * M, M * M * 4);
             }
         }
         float2 v[32];
@@ -350,6 +392,20 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
             }
             dft<32, -1>(v);
             P::p1_store(tid, E, v);
+        }
+        if (tid == 0) {
+            if (DYN) {
+                i_next = (int)gridDim.x + ticket;
+                if (i_next < A.K) {
+                    nxr = __ldg(A.pos + 2 * i_next);
+                    nxc = __ldg(A.pos + 2 * i_next + 1);
+                    prefetch_l2_bulk(A.c_in + (size_t)i_next * M * M, M * M * 8);
+                    if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)i_next * M * M, M * M * 4);
+                }
+            }
+            s_sched[4 * (par ^ 1)] = i_next;
+            s_sched[4 * (par ^ 1) + 1] = nxr;
+            s_sched[4 * (par ^ 1) + 2] = nxc;
         }
         __syncthreads();                                                     // barrier 1
         // ---------------- P2: DFT32 along the row ----------------------------------------------------------

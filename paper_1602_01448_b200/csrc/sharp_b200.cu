@@ -51,13 +51,14 @@ struct sharp_plan_s {
     int device = -1;         // CUDA device the plan was bound on
     int frame_ctas_max = 0;  // resident CTAs of the iteration kernel on that device
     int frame_nt = 256;
+    int sched_sel = 0;       // which of the two schedule counters the next frame launch uses
     int probe_chunk = 64, probe_nchunks = 0;
     int amp_blocks = 0;
 
     // workspace offsets
     size_t o_a = 0, o_c[2] = {0, 0}, o_psi_z = 0, o_psi_v[2] = {0, 0}, o_den = 0, o_cross = 0, o_w[4] = {0, 0, 0, 0}, o_scratch = 0,
            o_pos = 0, o_tile_ptr = 0, o_tile_frames = 0, o_partials = 0, o_err_partials = 0, o_err_sums = 0, o_pnum = 0,
-           o_pden = 0, o_scalars = 0, o_wtmp[3] = {0, 0, 0}, o_wcon = 0, o_pscal = 0, o_quads = 0, o_quad_sum = 0, o_num = 0, o_praw = 0, o_total = 0;
+           o_pden = 0, o_scalars = 0, o_wtmp[3] = {0, 0, 0}, o_wcon = 0, o_pscal = 0, o_quads = 0, o_quad_sum = 0, o_num = 0, o_praw = 0, o_sched = 0, o_total = 0;
 
     // state
     bool have_I = false, have_probe = false, have_frames = false, have_prev = false;
@@ -267,6 +268,10 @@ FrameArgs base_frame_args(sharp_plan_t *p)
     a.K = p->K;
     a.nr = p->nr;
     a.nc = p->nc;
+    // every frame launch consumes one schedule counter and zeroes the other for the launch after it
+    a.sched = p->dp<int>(p->o_sched) + p->sched_sel;
+    a.sched_next = p->dp<int>(p->o_sched) + (p->sched_sel ^ 1);
+    p->sched_sel ^= 1;
     return a;
 }
 
@@ -373,6 +378,28 @@ int free_probe_slot(const sharp_plan_t *p)
         if (j != p->w_cur && j != p->w_form && j != p->w_prev) return j;
     return -1;  // cannot happen: four buffers, three roles
 }
+
+// Every entry point that touches the device runs under the device the plan was bound on and restores the caller's
+// current device on return (a plan bound on cuda:1 may be driven while cuda:0 is current).
+struct DeviceScope {
+    int prev = -1;
+    explicit DeviceScope(const sharp_plan_t *p)
+    {
+        if (!p || !p->bound) return;
+        int cur = -1;
+        if (cudaGetDevice(&cur) == cudaSuccess && cur != p->device && cudaSetDevice(p->device) == cudaSuccess) prev = cur;
+    }
+    ~DeviceScope() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceScope(const DeviceScope &) = delete;
+    DeviceScope &operator=(const DeviceScope &) = delete;
+};
+
+// caller device pointers are read and written with 128-bit accesses
+bool misaligned(const void *ptr) { return reinterpret_cast<uintptr_t>(ptr) % 16 != 0; }
+#define CHECK_ALIGNED(ptr)                                                                              \
+    do {                                                                                                \
+        if ((ptr) != nullptr && misaligned(ptr)) return fail(p, SHARP_EINVAL, #ptr " must be 16-byte aligned"); \
+    } while (0)
 
 int check_ready(sharp_plan_t *p, bool need_I, bool need_probe)
 {
@@ -540,6 +567,7 @@ static int make_plan(sharp_plan_t **out, int m, int K, const int32_t *pos_rc, in
     p->o_quad_sum = take(4 * 8);
     p->o_num = take(p->nobj() * 8);            // raw object numerator of a sharded plan (summed over ranks in place)
     p->o_praw = take((size_t)m * m * 3 * 4);   // raw Eq. 10 sums (num.x, num.y, den) of a sharded plan
+    p->o_sched = take(2 * sizeof(int));        // frame counters of the dynamic schedule (frame_r.cuh)
     p->o_total = o;
     *out = p;
     return SHARP_OK;
@@ -583,9 +611,15 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
     p->ws = static_cast<unsigned char *>(dev_workspace);
     p->ws_bytes = bytes;
     p->stream = static_cast<cudaStream_t>(cuda_stream);
+    // the plan lives on the device that owns the workspace, whatever device is current now or later
+    cudaPointerAttributes pa;
+    CK(cudaPointerGetAttributes(&pa, dev_workspace));
+    if (pa.type != cudaMemoryTypeDevice) return fail(p, SHARP_EINVAL, "workspace is not device memory");
+    int dev = pa.device, sms = 0, prev_dev = -1;
+    CK(cudaGetDevice(&prev_dev));
+    struct Restore { int d; ~Restore() { if (d >= 0) cudaSetDevice(d); } } restore{prev_dev != dev ? prev_dev : -1};
+    if (prev_dev != dev) CK(cudaSetDevice(dev));
     // size the persistent grid from the occupancy of the iteration kernel
-    int dev = 0, sms = 0;
-    CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     int resident = 0, resident2 = 0;
     if (p->periodic) CK((frame_prepare_m<FRAME_ITER, true>(p->m, sms, &resident)));
@@ -606,6 +640,8 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
         CK(cudaMemcpyAsync(p->dp<int>(p->o_tile_frames), p->tile_frames.data(), p->tile_frames.size() * 4, cudaMemcpyHostToDevice, p->stream));
     CK(cudaMemsetAsync(p->dp<void>(p->o_scalars), 0, sizeof(DevScalars), p->stream));
     CK(cudaMemsetAsync(p->dp<void>(p->o_pscal), 0, sizeof(ProbeScalars), p->stream));
+    CK(cudaMemsetAsync(p->dp<void>(p->o_sched), 0, 2 * sizeof(int), p->stream));
+    p->sched_sel = 0;
     CK(cudaStreamSynchronize(p->stream));  // the host vectors may be read until here
     p->bound = true;
     p->have_I = p->have_probe = p->have_frames = p->have_prev = false;
@@ -619,7 +655,9 @@ int sharp_bind(sharp_plan_t *p, void *dev_workspace, size_t bytes, void *cuda_st
 
 int sharp_set_intensities(sharp_plan_t *p, const float *I_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
+    CHECK_ALIGNED(I_dev);
     if (!I_dev) return fail(p, SHARP_EINVAL, "I_dev is NULL");
     k_amplitudes<<<p->amp_blocks, 256, 0, p->stream>>>(p->m, p->K, I_dev, p->dp<float>(p->o_a), p->dp<double>(p->o_partials));
     CK_LAUNCH("k_amplitudes");
@@ -637,7 +675,9 @@ int sharp_set_intensities(sharp_plan_t *p, const float *I_dev)
 
 int sharp_set_probe(sharp_plan_t *p, const float *w_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
+    CHECK_ALIGNED(w_dev);
     if (!w_dev) return fail(p, SHARP_EINVAL, "w_dev is NULL");
     const size_t bytes = (size_t)p->m * p->m * 8;
     if (!p->have_frames) {
@@ -658,7 +698,9 @@ int sharp_set_probe(sharp_plan_t *p, const float *w_dev)
 
 int sharp_set_object(sharp_plan_t *p, const float *psi_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(psi_dev);
     p->cur = 0; p->vcur = 0;
     k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc,
                                                             reinterpret_cast<const float2 *>(psi_dev),
@@ -669,7 +711,9 @@ int sharp_set_object(sharp_plan_t *p, const float *psi_dev)
 
 int sharp_set_frames(sharp_plan_t *p, const float *z_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(z_dev);
     if (!z_dev) return fail(p, SHARP_EINVAL, "z_dev is NULL");
     p->cur = 0; p->vcur = 0;
     CK(cudaMemcpyAsync(p->dp<void>(p->o_c[0]), z_dev, p->npx() * 8, cudaMemcpyDeviceToDevice, p->stream));
@@ -695,6 +739,7 @@ int sharp_set_probe_refine(sharp_plan_t *p, int every)
 
 int sharp_iterate(sharp_plan_t *p, int n, float beta)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, true, true)) return rc;
     if (n < 0) return fail(p, SHARP_EINVAL, "n must be >= 0");
     if (!(beta > 0.5f && beta <= 1.0f)) return fail(p, SHARP_EINVAL, "beta must be in (0.5, 1] (PAPER.md:178), got %g", (double)beta);
@@ -778,7 +823,9 @@ int sharp_iterate(sharp_plan_t *p, int n, float beta)
 
 int sharp_get_object(sharp_plan_t *p, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(out_dev);
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet (call sharp_set_object or sharp_iterate)");
     if (int rc = ensure_object_state(p)) return rc;
@@ -788,7 +835,9 @@ int sharp_get_object(sharp_plan_t *p, float *out_dev)
 
 int sharp_get_probe(sharp_plan_t *p, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(out_dev);
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     CK(cudaMemcpyAsync(out_dev, p->dp<void>(p->o_w[p->w_cur]), (size_t)p->m * p->m * 8, cudaMemcpyDeviceToDevice, p->stream));
     return SHARP_OK;
@@ -796,7 +845,9 @@ int sharp_get_probe(sharp_plan_t *p, float *out_dev)
 
 int sharp_get_frames(sharp_plan_t *p, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(out_dev);
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
     k_materialize<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc, p->dp<float2>(p->o_c[p->cur]),
@@ -808,7 +859,9 @@ int sharp_get_frames(sharp_plan_t *p, float *out_dev)
 
 int sharp_get_amplitudes(sharp_plan_t *p, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, true, false)) return rc;
+    CHECK_ALIGNED(out_dev);
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     k_amplitudes_natural<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<float>(p->o_a), out_dev);
     CK_LAUNCH("k_amplitudes_natural");
@@ -817,6 +870,7 @@ int sharp_get_amplitudes(sharp_plan_t *p, float *out_dev)
 
 int sharp_errors(sharp_plan_t *p, float out[3])
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, true, true)) return rc;
     if (!out) return fail(p, SHARP_EINVAL, "out is NULL");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
@@ -848,6 +902,7 @@ int sharp_errors(sharp_plan_t *p, float out[3])
 
 int sharp_sync(sharp_plan_t *p)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
     CK(cudaStreamSynchronize(p->stream));
     return SHARP_OK;
@@ -858,6 +913,7 @@ long long sharp_launch_count(const sharp_plan_t *p) { return p ? p->launches : 0
 
 int sharp_profile(sharp_plan_t *p, int on)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
     CK(cudaStreamSynchronize(p->stream));
     for (auto &s : p->prof) { cudaEventDestroy(s.beg); cudaEventDestroy(s.end); }
@@ -868,6 +924,7 @@ int sharp_profile(sharp_plan_t *p, int on)
 
 int sharp_profile_read(sharp_plan_t *p, double ms[SHARP_PROF_NCLASS], long long launches[SHARP_PROF_NCLASS])
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
     if (!ms || !launches) return fail(p, SHARP_EINVAL, "NULL argument");
     CK(cudaStreamSynchronize(p->stream));
@@ -923,7 +980,9 @@ int sharp_cover_counts(const sharp_plan_t *p, int32_t *out_host)
 
 int sharp_frame_index(sharp_plan_t *p, long long *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
+    CHECK_ALIGNED(out_dev);
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     k_frame_index<<<grid_for(p->npx()), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc, out_dev);
     CK_LAUNCH("k_frame_index");
@@ -932,7 +991,10 @@ int sharp_frame_index(sharp_plan_t *p, long long *out_dev)
 
 int sharp_op_split(sharp_plan_t *p, const float *psi_dev, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(psi_dev);
+    CHECK_ALIGNED(out_dev);
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     k_split<<<grid_for(p->npx() / 2), 256, 0, p->stream>>>(p->m, p->K, p->dp<int>(p->o_pos), p->nr, p->nc, reinterpret_cast<const float2 *>(psi_dev),
                                                             p->dp<float2>(p->o_w[p->w_cur]), reinterpret_cast<float2 *>(out_dev));
@@ -942,7 +1004,10 @@ int sharp_op_split(sharp_plan_t *p, const float *psi_dev, float *out_dev)
 
 int sharp_op_overlap(sharp_plan_t *p, const float *f_dev, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(f_dev);
+    CHECK_ALIGNED(out_dev);
     if (!f_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
     if (int rc = ensure_object_state(p)) return rc;
     OverlapArgs a = base_overlap_args(p);
@@ -954,7 +1019,10 @@ int sharp_op_overlap(sharp_plan_t *p, const float *f_dev, float *out_dev)
 
 int sharp_op_pa(sharp_plan_t *p, const float *f_dev, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, true, false)) return rc;
+    CHECK_ALIGNED(f_dev);
+    CHECK_ALIGNED(out_dev);
     if (!f_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
     FrameArgs fa = base_frame_args(p);
     fa.c_in = reinterpret_cast<const float2 *>(f_dev);
@@ -966,7 +1034,10 @@ int sharp_op_pa(sharp_plan_t *p, const float *f_dev, float *out_dev)
 
 int sharp_op_fft2(sharp_plan_t *p, const float *f_dev, float *out_dev, int sign)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
+    CHECK_ALIGNED(f_dev);
+    CHECK_ALIGNED(out_dev);
     if (!f_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
     if (f_dev == out_dev) return fail(p, SHARP_EINVAL, "sharp_op_fft2 is out of place");
     if (sign != 1 && sign != -1) return fail(p, SHARP_EINVAL, "sign must be -1 (F) or +1 (F*)");
@@ -979,7 +1050,11 @@ int sharp_op_fft2(sharp_plan_t *p, const float *f_dev, float *out_dev, int sign)
 
 int sharp_op_probe(sharp_plan_t *p, const float *psi_dev, const float *z_dev, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(psi_dev);
+    CHECK_ALIGNED(z_dev);
+    CHECK_ALIGNED(out_dev);
     if (!psi_dev || !z_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
     const int mm_i = p->m * p->m;
     dim3 g(mm_i / 256, p->probe_nchunks);
@@ -996,6 +1071,7 @@ int sharp_op_probe(sharp_plan_t *p, const float *psi_dev, const float *z_dev, fl
 int sharp_reconstruct_host(sharp_plan_t *p, const float *I_host, const float *w_host, int n, float beta,
                            float *psi_out_host, float *w_out_host, float eps_out[3])
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
     if (!I_host || !w_host) return fail(p, SHARP_EINVAL, "NULL input");
     if (n < 0 || !(beta > 0.5f && beta <= 1.0f)) return fail(p, SHARP_EINVAL, "bad n or beta");
@@ -1020,7 +1096,10 @@ int sharp_reconstruct_host(sharp_plan_t *p, const float *I_host, const float *w_
 // ---- eps_0 against a known solution, default initialisations ----------------------------------
 int sharp_eps0(sharp_plan_t *p, const float *psi0_dev, const float *w0_dev, float *out_host)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
+    CHECK_ALIGNED(psi0_dev);
+    CHECK_ALIGNED(w0_dev);
     if (!psi0_dev || !out_host) return fail(p, SHARP_EINVAL, "NULL argument");
     if (!p->have_frames) return fail(p, SHARP_ESTATE, "no frames yet");
     if (int rc = ensure_object_state(p)) return rc;
@@ -1048,6 +1127,7 @@ int sharp_eps0(sharp_plan_t *p, const float *psi0_dev, const float *w0_dev, floa
 
 int sharp_init_probe(sharp_plan_t *p)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, true, false)) return rc;
     const int mm = p->m * p->m;
     double *part = p->dp<double>(p->o_pnum);                // probe_nchunks * m * m * 8 bytes
@@ -1067,7 +1147,9 @@ int sharp_init_probe(sharp_plan_t *p)
 
 int sharp_op_random_object(sharp_plan_t *p, unsigned long long seed, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
+    CHECK_ALIGNED(out_dev);
     if (!out_dev) return fail(p, SHARP_EINVAL, "out_dev is NULL");
     k_random_object<<<grid_for(p->nobj()), 256, 0, p->stream>>>(p->nobj(), seed, reinterpret_cast<float2 *>(out_dev));
     CK_LAUNCH("k_random_object");
@@ -1076,6 +1158,7 @@ int sharp_op_random_object(sharp_plan_t *p, unsigned long long seed, float *out_
 
 int sharp_init_object_random(sharp_plan_t *p, unsigned long long seed)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, true)) return rc;
     // psi_v[1] is free here: sharp_set_object resets the factored state (psi_v = 0) before anything reads it
     float *tmp = p->dp<float>(p->o_psi_v[1]);
@@ -1099,7 +1182,9 @@ int sharp_set_sharded(sharp_plan_t *p, sharp_allreduce_fn fn, void *user, long l
 // ---- illumination constraints and re-centring --------------------------------------------------
 int sharp_set_probe_constraint(sharp_plan_t *p, int kind, const float *con_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
+    CHECK_ALIGNED(con_dev);
     if (kind < 0 || kind > 2) return fail(p, SHARP_EINVAL, "constraint kind must be 0 (none), 1 (mask) or 2 (amplitude)");
     if (kind != 0 && !con_dev) return fail(p, SHARP_EINVAL, "con_dev is NULL");
     const int mm = p->m * p->m;
@@ -1114,6 +1199,7 @@ int sharp_set_probe_constraint(sharp_plan_t *p, int kind, const float *con_dev)
 
 int sharp_set_probe_recentre(sharp_plan_t *p, int on)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
     p->probe_recentre = on != 0;
     CK(cudaMemsetAsync(p->dp<ProbeScalars>(p->o_pscal)->shift, 0, 4 * sizeof(int), p->stream));
@@ -1122,6 +1208,7 @@ int sharp_set_probe_recentre(sharp_plan_t *p, int on)
 
 int sharp_get_probe_shift(sharp_plan_t *p, int32_t last[2], int32_t total[2])
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
     ProbeScalars ps;
     CK(cudaMemcpyAsync(&ps, p->dp<void>(p->o_pscal), sizeof ps, cudaMemcpyDeviceToHost, p->stream));
@@ -1133,7 +1220,10 @@ int sharp_get_probe_shift(sharp_plan_t *p, int32_t last[2], int32_t total[2])
 
 int sharp_op_probe_constrain(sharp_plan_t *p, const float *w_dev, float *out_dev)
 {
+    DeviceScope dev_scope(p);
     if (int rc = check_ready(p, false, false)) return rc;
+    CHECK_ALIGNED(w_dev);
+    CHECK_ALIGNED(out_dev);
     if (!w_dev || !out_dev) return fail(p, SHARP_EINVAL, "NULL argument");
     if (w_dev == out_dev) return fail(p, SHARP_EINVAL, "sharp_op_probe_constrain is out of place");
     return constrain_probe(p, reinterpret_cast<const float2 *>(w_dev), reinterpret_cast<float2 *>(out_dev));

@@ -266,3 +266,24 @@ def test_periodic_fixed_point_and_blind_step(pscan, oracle):
     assert rel(rec.get_probe().cpu().numpy(), o.w) < 3e-5
     rec.set_probe_refine(0)
     rec.set_probe(pscan["wt"])
+
+
+# ---- boundary behaviour ---------------------------------------------------------------------------------------------
+def test_misaligned_device_pointers_are_refused(scan):
+    """The kernels use 128-bit accesses: a caller pointer that is only 8-byte aligned (a complex64 view with an odd
+    storage offset) is SHARP_EINVAL, not a misaligned-address fault."""
+    import torch
+    cfg, rec = scan["cfg"], scan["rec"]
+    m = cfg.m
+    buf = torch.zeros(m * m + 1, dtype=torch.complex64, device="cuda")
+    odd = buf[1:]
+    assert odd.data_ptr() % 16 == 8 and odd.is_contiguous()
+    with pytest.raises(sharp.SharpError) as e:
+        rec.set_probe(odd)
+    assert e.value.code == sharp.SHARP_EINVAL
+    big = torch.zeros(cfg.K * m * m + 1, dtype=torch.complex64, device="cuda")
+    with pytest.raises(sharp.SharpError) as e:
+        rec.op_pa(big[1:])
+    assert e.value.code == sharp.SHARP_EINVAL
+    rec.set_probe(scan["wt"])                      # the plan is still usable
+    assert np.isfinite(rec.get_probe().cpu().numpy()).all()
