@@ -93,6 +93,108 @@ __device__ __forceinline__ void cluster_barrier()
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
+// ---- arithmetic both frame kernels share (written once) --------------------------------------------------------------
+// Magnitude projection fused with the frame half of RAAR, on 8 Fourier coefficients x[] (un-normalised transform) with
+// their amplitudes av[] = a/m:  C^ = Z^ (beta/m^2 + (1 - 2 beta)(a/m)/|Z^|);  |Z^|^2 <= thr2 takes the phase as 1 (reading G4).
+__device__ __forceinline__ void frame_project8(float2 *x, const float *av, float thr2, float bm, float om)
+{
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const float mag2 = x[k].x * x[k].x + x[k].y * x[k].y;
+        const float oa = om * av[k];
+        if (mag2 > thr2) {
+            const float sc = fmaf(oa, rsqrtf(mag2), bm);
+            x[k].x *= sc;
+            x[k].y *= sc;
+        } else {
+            x[k].x = fmaf(bm, x[k].x, oa);
+            x[k].y = bm * x[k].y;
+        }
+    }
+}
+
+// sum over a thread's 32 coefficients of |a - |F z||^2 (= |P_a z - z|^2 by Parseval; G4 branch: |a - F z|^2); ap points at
+// the thread's first amplitude, consecutive registers are 32 floats apart
+template <int M>
+__device__ __forceinline__ float frame_err_a32(const float2 *v, const float *ap, float thr2)
+{
+    const float fm = (float)M, inv_m = 1.0f / (float)M;
+    float sa = 0.f;
+#pragma unroll
+    for (int q = 0; q < 32; ++q) {
+        const float a = __ldcs(ap + q * 32) * fm;
+        const float mag2 = v[q].x * v[q].x + v[q].y * v[q].y;
+        if (mag2 > thr2) {
+            const float d = a - sqrtf(mag2) * inv_m;
+            sa += d * d;
+        } else {
+            const float dx = a - v[q].x * inv_m, dy = v[q].y * inv_m;
+            sa += dx * dx + dy * dy;
+        }
+    }
+    return sa;
+}
+
+// |P_Q z - z|^2 and |z - z_prev|^2 over a thread's 32 frame pixels (rows r_lo + NLO k of column col); v[] holds z
+template <int M, int NLO>
+__device__ __forceinline__ void frame_err_qd32(const FrameArgs &A, const float2 *v, size_t fbase, int xr, int xc, int r_lo, int col,
+                                                float &sq, float &sd)
+{
+    sq = 0.f;
+    sd = 0.f;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        const int r = r_lo + NLO * k;
+        int prw = xr + r, pcw = xc + col;      // modulo the image size (identity without the periodic boundary)
+        if (prw >= A.nr) prw -= A.nr;
+        if (pcw >= A.nc) pcw -= A.nc;
+        const size_t op = (size_t)prw * A.nc + pcw;
+        const float2 d = csub(cmul(__ldg(A.w_cur + r * M + col), __ldg(A.psi_z + op)), v[k]);
+        sq += d.x * d.x + d.y * d.y;
+        float2 zp = make_float2(0.f, 0.f);
+        if (A.c_prev != nullptr) {
+            zp = ld_stream(A.c_prev + fbase + (size_t)r * M + col);
+            if (A.psi_v_prev != nullptr) zp = cadd(zp, cmul(__ldg(A.w_form_prev + r * M + col), __ldg(A.psi_v_prev + op)));
+        }
+        const float2 dd = csub(v[k], zp);
+        sd += dd.x * dd.x + dd.y * dd.y;
+    }
+}
+
+// deterministic reduction of the three residual sums of a CTA: fixed xor-tree inside each warp (shuffles), then the
+// warp sums in warp order by thread 0; one triple per CTA
+__device__ __forceinline__ void frame_err_reduce(double s_a, double s_q, double s_d, unsigned char *smem_raw, int nwarps,
+                                                  double *err_partials)
+{
+    const int tid = threadIdx.x, wq = tid >> 5, lane = tid & 31;
+    __syncthreads();
+    double *red = reinterpret_cast<double *>(smem_raw);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        s_a += __shfl_xor_sync(0xffffffffu, s_a, off);
+        s_q += __shfl_xor_sync(0xffffffffu, s_q, off);
+        s_d += __shfl_xor_sync(0xffffffffu, s_d, off);
+    }
+    if (lane == 0) {
+        red[3 * wq + 0] = s_a;
+        red[3 * wq + 1] = s_q;
+        red[3 * wq + 2] = s_d;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double a = 0.0, q = 0.0, d = 0.0;
+        for (int w = 0; w < nwarps; ++w) {
+            a += red[3 * w + 0];
+            q += red[3 * w + 1];
+            d += red[3 * w + 2];
+        }
+        err_partials[3 * blockIdx.x + 0] = a;
+        err_partials[3 * blockIdx.x + 1] = q;
+        err_partials[3 * blockIdx.x + 2] = d;
+    }
+}
+
 #endif  // __CUDACC__
+
 
 }  // namespace sharp

@@ -368,25 +368,8 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
                 }
             }
             if constexpr (MODE == FRAME_ERR) {
-                float sq = 0.f, sd = 0.f;
-#pragma unroll
-                for (int k = 0; k < 32; ++k) {
-                    const int r = r_lo + NLO * k;
-                    int prw = xr + r, pcw = xc + col;      // modulo the image size (identity without the periodic boundary)
-                    if (prw >= A.nr) prw -= A.nr;
-                    if (pcw >= A.nc) pcw -= A.nc;
-                    const size_t op = (size_t)prw * A.nc + pcw;
-                    const float2 d = csub(cmul(__ldg(A.w_cur + r * M + col), __ldg(A.psi_z + op)), v[k]);
-                    sq += d.x * d.x + d.y * d.y;
-                    float2 zp = make_float2(0.f, 0.f);
-                    if (A.c_prev != nullptr) {
-                        zp = ld_stream(A.c_prev + fbase + (size_t)r * M + col);
-                        if (A.psi_v_prev != nullptr)
-                            zp = cadd(zp, cmul(__ldg(A.w_form_prev + r * M + col), __ldg(A.psi_v_prev + op)));
-                    }
-                    const float2 dd = csub(v[k], zp);
-                    sd += dd.x * dd.x + dd.y * dd.y;
-                }
+                float sq, sd;
+                frame_err_qd32<M, NLO>(A, v, fbase, xr, xc, r_lo, col, sq, sd);
                 s_q += (double)sq;
                 s_d += (double)sd;
             }
@@ -433,21 +416,7 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
         } else {
             const float *ap = A.a_int + fbase + (size_t)(wq * 32) * 32 + lane;
             if constexpr (MODE == FRAME_ERR) {
-                const float fm = (float)M, inv_m = 1.0f / (float)M;
-                float sa = 0.f;
-#pragma unroll
-                for (int q = 0; q < 32; ++q) {
-                    const float a = __ldcs(ap + q * 32) * fm;
-                    const float mag2 = v[q].x * v[q].x + v[q].y * v[q].y;
-                    if (mag2 > thr2) {
-                        const float d = a - sqrtf(mag2) * inv_m;
-                        sa += d * d;
-                    } else {
-                        const float dx = a - v[q].x * inv_m, dy = v[q].y * inv_m;
-                        sa += dx * dx + dy * dy;
-                    }
-                }
-                s_a += (double)sa;
+                s_a += (double)frame_err_a32<M>(v, ap, thr2);
                 __syncthreads();
                 continue;
             } else {
@@ -456,20 +425,7 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
                     float av[8];
 #pragma unroll
                     for (int k = 0; k < 8; ++k) av[k] = __ldcs(ap + (q0 + k) * 32);
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        float2 &x = v[q0 + k];
-                        const float mag2 = x.x * x.x + x.y * x.y;
-                        const float oa = om * av[k];
-                        if (mag2 > thr2) {
-                            const float sc = fmaf(oa, rsqrtf(mag2), bm);
-                            x.x *= sc;
-                            x.y *= sc;
-                        } else {
-                            x.x = fmaf(bm, x.x, oa);
-                            x.y = bm * x.y;
-                        }
-                    }
+                    frame_project8(v + q0, av, thr2, bm, om);
                 }
             }
         }
@@ -498,35 +454,7 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
         if (wq == 0) r_tmem_dealloc(*reinterpret_cast<volatile unsigned *>(tmem_slot), 256);
     }
 
-    if constexpr (MODE == FRAME_ERR) {
-        // deterministic reduction of the three sums: fixed xor-tree inside each warp (shuffles), then the warp sums
-        // in warp order by thread 0; one triple per CTA
-        __syncthreads();
-        double *red = reinterpret_cast<double *>(smem_raw);
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            s_a += __shfl_xor_sync(0xffffffffu, s_a, off);
-            s_q += __shfl_xor_sync(0xffffffffu, s_q, off);
-            s_d += __shfl_xor_sync(0xffffffffu, s_d, off);
-        }
-        if (lane == 0) {
-            red[3 * wq + 0] = s_a;
-            red[3 * wq + 1] = s_q;
-            red[3 * wq + 2] = s_d;
-        }
-        __syncthreads();
-        if (tid == 0) {
-            double a = 0.0, q = 0.0, d = 0.0;
-            for (int w = 0; w < C::NW; ++w) {
-                a += red[3 * w + 0];
-                q += red[3 * w + 1];
-                d += red[3 * w + 2];
-            }
-            A.err_partials[3 * blockIdx.x + 0] = a;
-            A.err_partials[3 * blockIdx.x + 1] = q;
-            A.err_partials[3 * blockIdx.x + 2] = d;
-        }
-    }
+    if constexpr (MODE == FRAME_ERR) frame_err_reduce(s_a, s_q, s_d, smem_raw, C::NW, A.err_partials);
 }
 
 #endif  // __CUDACC__

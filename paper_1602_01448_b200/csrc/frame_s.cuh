@@ -34,6 +34,10 @@
 #include "fft_regs.cuh"
 #include "frame_common.cuh"
 
+#ifndef SHARP_STAGGER_S_NS
+#define SHARP_STAGGER_S_NS 0
+#endif
+
 namespace sharp {
 
 template <int M, int NT_>
@@ -246,6 +250,16 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
     const float bm = A.bm, om = A.om;
     double s_a = 0.0, s_q = 0.0, s_d = 0.0;
 
+#if SHARP_STAGGER_S_NS > 0
+    // clusters started in phases (see frame_r.cuh: all SMs in lockstep run their HBM bursts at the same time)
+    if (MODE == FRAME_ITER && A.K > 2 * nclusters) {
+        const unsigned delay = ((unsigned)cid % 8u) * (unsigned)(SHARP_STAGGER_S_NS * (M / 256) * (M / 256));
+        unsigned long long t0, t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+        do { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); } while (t1 - t0 < delay);
+    }
+#endif
+
     for (int i = cid; i < A.K; i += nclusters) {
         const int xr = __ldg(A.pos + 2 * i), xc = __ldg(A.pos + 2 * i + 1);
         const size_t fbase = (size_t)i * M * M;
@@ -288,25 +302,8 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
                     }
                 }
                 if constexpr (MODE == FRAME_ERR) {
-                    float sq = 0.f, sd = 0.f;
-#pragma unroll
-                    for (int k = 0; k < 32; ++k) {
-                        const int r = r_lo + NLO * k;
-                        int prw = xr + r, pcw = xc + col;   // modulo the image size (identity without the periodic boundary)
-                        if (prw >= A.nr) prw -= A.nr;
-                        if (pcw >= A.nc) pcw -= A.nc;
-                        const size_t op = (size_t)prw * A.nc + pcw;
-                        const float2 d = csub(cmul(__ldg(A.w_cur + r * M + col), __ldg(A.psi_z + op)), v[k]);
-                        sq += d.x * d.x + d.y * d.y;
-                        float2 zp = make_float2(0.f, 0.f);
-                        if (A.c_prev != nullptr) {
-                            zp = ld_stream(A.c_prev + fbase + (size_t)r * M + col);
-                            if (A.psi_v_prev != nullptr)
-                                zp = cadd(zp, cmul(__ldg(A.w_form_prev + r * M + col), __ldg(A.psi_v_prev + op)));
-                        }
-                        const float2 dd = csub(v[k], zp);
-                        sd += dd.x * dd.x + dd.y * dd.y;
-                    }
+                    float sq, sd;
+                    frame_err_qd32<M, NLO>(A, v, fbase, xr, xc, r_lo, col, sq, sd);
                     s_q += (double)sq;
                     s_d += (double)sd;
                 }
@@ -359,42 +356,10 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
             } else {
                 const float *ap = A.a_int + fbase + (size_t)(uhi * 32) * 32 + lane;
                 if constexpr (MODE == FRAME_ERR) {
-                    const float fm = (float)M, inv_m = 1.0f / (float)M;
-                    float sa = 0.f;
-#pragma unroll
-                    for (int q = 0; q < 32; ++q) {
-                        const float a = __ldcs(ap + q * 32) * fm;
-                        const float mag2 = v[q].x * v[q].x + v[q].y * v[q].y;
-                        if (mag2 > thr2) {
-                            const float d = a - sqrtf(mag2) * inv_m;
-                            sa += d * d;
-                        } else {
-                            const float dx = a - v[q].x * inv_m, dy = v[q].y * inv_m;
-                            sa += dx * dx + dy * dy;
-                        }
-                    }
-                    s_a += (double)sa;
+                    s_a += (double)frame_err_a32<M>(v, ap, thr2);
                 } else {
 #pragma unroll
-                    for (int q0 = 0; q0 < 32; q0 += 8) {
-                        float av[8];
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) av[k] = av_all[q0 + k];
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) {
-                            float2 &x = v[q0 + k];
-                            const float mag2 = x.x * x.x + x.y * x.y;
-                            const float oa = om * av[k];
-                            if (mag2 > thr2) {
-                                const float sc = fmaf(oa, rsqrtf(mag2), bm);
-                                x.x *= sc;
-                                x.y *= sc;
-                            } else {
-                                x.x = fmaf(bm, x.x, oa);
-                                x.y = bm * x.y;
-                            }
-                        }
-                    }
+                    for (int q0 = 0; q0 < 32; q0 += 8) frame_project8(v + q0, av_all + q0, thr2, bm, om);
                     P::template p4_math<true>(tid, tw, v);
                     P::x3_store_rows(tid, E, v);
                     __syncwarp();
@@ -426,34 +391,7 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
         }
     }
 
-    if constexpr (MODE == FRAME_ERR) {
-        // deterministic reduction: fixed xor-tree inside each warp, then the warp sums in warp order; one triple per CTA
-        __syncthreads();
-        double *red = reinterpret_cast<double *>(smem_raw);
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            s_a += __shfl_xor_sync(0xffffffffu, s_a, off);
-            s_q += __shfl_xor_sync(0xffffffffu, s_q, off);
-            s_d += __shfl_xor_sync(0xffffffffu, s_d, off);
-        }
-        if (lane == 0) {
-            red[3 * wq + 0] = s_a;
-            red[3 * wq + 1] = s_q;
-            red[3 * wq + 2] = s_d;
-        }
-        __syncthreads();
-        if (tid == 0) {
-            double a = 0.0, q = 0.0, d = 0.0;
-            for (int w = 0; w < C::NW; ++w) {
-                a += red[3 * w + 0];
-                q += red[3 * w + 1];
-                d += red[3 * w + 2];
-            }
-            A.err_partials[3 * blockIdx.x + 0] = a;
-            A.err_partials[3 * blockIdx.x + 1] = q;
-            A.err_partials[3 * blockIdx.x + 2] = d;
-        }
-    }
+    if constexpr (MODE == FRAME_ERR) frame_err_reduce(s_a, s_q, s_d, smem_raw, C::NW, A.err_partials);
 }
 
 #endif  // __CUDACC__

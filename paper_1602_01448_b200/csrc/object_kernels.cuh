@@ -409,6 +409,8 @@ __global__ void __launch_bounds__(256) k_probe_partial(int m, int K, int chunk, 
                                                         const float2 *c, const float2 *psi_v, const float2 *w_form,
                                                         const float2 *psi, float2 *pnum, float *pden)
 {
+    // one frame in flight per thread at 32 registers and full occupancy: measured 87 us at config 3; four frames in
+    // flight with the chunk's positions staged in shared memory (55 registers, half the warps) 94 us
     const int pix = blockIdx.x * blockDim.x + threadIdx.x;  // m*m is a multiple of 256
     const int r = pix / m, col = pix % m;
     const int i0 = blockIdx.y * chunk, i1 = min(K, i0 + chunk);
