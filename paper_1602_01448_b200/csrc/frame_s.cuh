@@ -24,7 +24,8 @@
 //
 // Measured at config-4 size (1,600 frames, us per launch): 256-thread CTAs in clusters of 4: 1098; 128-thread CTAs
 // (m = 256: strips of 16 columns, four CTAs per SM) in clusters of 8: 929, in clusters of 4: 1212; the probe parked in
-// tensor memory (4 x 128 columns per SM): 1821 (the allocations of the four resident CTAs serialise), dropped.
+// tensor memory (4 x 128 columns per SM): 1821 (the allocations of the four resident CTAs serialise), dropped.  Clusters
+// started in phases (what helps frame_r.cuh): 863 without, 863 / 869 with 8 phases of 2.5 / 5 us: no effect, dropped.
 // A bulk L2 prefetch of the cluster's next frame (what frame_r.cuh does) costs here: 926 with, 865 without (config 5:
 // 5.45 / 4.99 ms): the prefetched frames push the scratch frames out of L2.
 // The scratch frame (m^2 c64 per cluster) is the only data that leaves the SM between F and F*; it is re-used for
@@ -33,10 +34,6 @@
 #pragma once
 #include "fft_regs.cuh"
 #include "frame_common.cuh"
-
-#ifndef SHARP_STAGGER_S_NS
-#define SHARP_STAGGER_S_NS 0
-#endif
 
 namespace sharp {
 
@@ -249,16 +246,6 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
     const float thr2 = A.sc->thr2;
     const float bm = A.bm, om = A.om;
     double s_a = 0.0, s_q = 0.0, s_d = 0.0;
-
-#if SHARP_STAGGER_S_NS > 0
-    // clusters started in phases (see frame_r.cuh: all SMs in lockstep run their HBM bursts at the same time)
-    if (MODE == FRAME_ITER && A.K > 2 * nclusters) {
-        const unsigned delay = ((unsigned)cid % 8u) * (unsigned)(SHARP_STAGGER_S_NS * (M / 256) * (M / 256));
-        unsigned long long t0, t1;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
-        do { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); } while (t1 - t0 < delay);
-    }
-#endif
 
     for (int i = cid; i < A.K; i += nclusters) {
         const int xr = __ldg(A.pos + 2 * i), xc = __ldg(A.pos + 2 * i + 1);

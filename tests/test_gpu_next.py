@@ -287,3 +287,36 @@ def test_misaligned_device_pointers_are_refused(scan):
     assert e.value.code == sharp.SHARP_EINVAL
     rec.set_probe(scan["wt"])                      # the plan is still usable
     assert np.isfinite(rec.get_probe().cpu().numpy()).all()
+
+
+def test_deferred_and_flushed_blind_paths_agree(scan, oracle):
+    """After an illumination update the library defers Q*Q, the cross term and the re-gathered object estimate to the next
+    iteration's overlap pass (OV_BLIND); any reader (errors, get_object, eps0) flushes them at once instead.  Both orders
+    must give the oracle's state."""
+    cfg, rec = scan["cfg"], scan["rec"]
+    m = cfg.m
+    z0 = (synth.exit_waves(cfg, scan["obj"], scan["w0"], scan["pos"]) * (1 + 0.2 * _rc((cfg.K, m, m), 91))).astype(np.complex64)
+    o = oracle.Oracle(m, scan["pos"], scan["shape"], scan["I"], scan["w0"], refine_every=1)
+    o.set_frames(z0)
+    o.iterate(3, cfg.beta)
+    runs = []
+    for flush in (False, True):
+        rec.set_probe(scan["w0"])
+        rec.set_probe_refine(1)
+        rec.set_frames(z0)
+        if flush:
+            for _ in range(3):
+                rec.iterate(1, cfg.beta)
+                rec.errors(); rec.get_object()             # forces OV_DEN + OV_REGATHER right after every update
+        else:
+            rec.iterate(3, cfg.beta)                        # two OV_BLIND passes inside
+        runs.append((rec.get_frames().cpu().numpy(), rec.get_probe().cpu().numpy(), rec.errors(), rec.get_object().cpu().numpy()))
+    for z, w, eps, psi in runs:
+        assert rel(z, o.z) < 5e-5 and rel(w, o.w) < 5e-5
+        assert np.allclose(eps, o.errors(), rtol=EPS_TOL)
+    assert rel(runs[0][0], runs[1][0]) < 2e-5
+    den = oracle.overlap_den(o.w, scan["pos"], scan["shape"])
+    lit = den >= 1e-3 * den.max()
+    assert rel(runs[0][3][lit], runs[1][3][lit]) < 2e-5 and rel(runs[0][3][lit], o.object()[lit]) < 5e-5
+    rec.set_probe_refine(0)
+    rec.set_probe(scan["wt"])
