@@ -241,17 +241,27 @@ __device__ __forceinline__ void object_epilogue(const OverlapArgs &A, size_t p, 
 // constant ty M + tx), and the range of tile rows / columns the frame covers, packed in one word.  UNR frames are in
 // flight per thread at a time and are accumulated in list order (ascending frame index: reading G17).
 #ifndef SHARP_OV_UNR
-#define SHARP_OV_UNR 6
+#define SHARP_OV_UNR 3
+#endif
+#ifndef SHARP_OVB_UNR          // OV_BLIND: four arrays per (frame, row) pair
+#define SHARP_OVB_UNR 1
+#endif
+#ifndef SHARP_OVB_MINB
+#define SHARP_OVB_MINB 3
 #endif
 #ifndef SHARP_OV_MINB
-#define SHARP_OV_MINB 2
+#define SHARP_OV_MINB 4
 #endif
-// The explicit minimum of resident CTAs matters beyond occupancy: with __launch_bounds__(256) alone ptxas (12.9) allocates
-// 39 registers and interleaves every pair of loads with the arithmetic that consumes it (one frame row in flight per
-// thread); with a minimum given it batches 12-14 loads as written (56 registers).  Measured at config 2 (us per launch):
-// 131 without; UNR 4 / min 3: 104.6; 4 / 4: 104.8; 8 / 3: 104.4; 6 / 2: 101.1.
+// Two things decide how many loads ptxas (12.9) keeps in flight here, and both were found the hard way:
+//  - with __launch_bounds__(256) alone it allocates 39 registers and interleaves every pair of loads with the arithmetic that
+//    consumes it; with a minimum CTA count given it batches the loads as written;
+//  - arithmetic predicated with the same condition as its loads keeps one of the 7 predicate registers live per (frame, row)
+//    pair, which caps a batch at 6-7 pairs; out-of-range pairs are therefore loaded as zeros and accumulated unconditionally.
+// Measured at config 2 (us per launch; UNR frames per batch / minimum CTAs): predicated 4/3 104.6, 6/2 101.1; unconditional
+// 4/2 123, 6/2 118, 4/3 99.1, 2/4 94.5, 2/5 94.6, 3/4 91.6 (kept), 3/5 132, 2/6 112, 1/8 117: occupancy (32 warps) buys more
+// than a longer batch per thread.  OV_BLIND (config 3): 2/2 176.8, 1/3 170.6 (kept), 1/4 169.0, 2/3 232, 1/2 215.
 template <int M, int MODE>
-__global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
+__global__ void __launch_bounds__(256, MODE == OV_BLIND ? SHARP_OVB_MINB : SHARP_OV_MINB) k_overlap(OverlapArgs A)
 {
     const int tile = blockIdx.x;
     const int tr = tile / A.tiles_c, tc = tile % A.tiles_c;
@@ -271,7 +281,7 @@ __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
         dn[k] = 0.f;
     }
 
-    constexpr int CH = 128, UNR = (MODE == OV_BLIND) ? 2 : SHARP_OV_UNR;
+    constexpr int CH = 128, UNR = (MODE == OV_BLIND) ? SHARP_OVB_UNR : SHARP_OV_UNR;
     __shared__ long long s_foff[CH];     // fi M^2 + (tile row0 - x_r) M + (tile col0 - x_c): may be negative before toff is added
     __shared__ int s_woff[CH];           // the same without the frame term
     __shared__ unsigned s_rng[CH];       // r_lo | r_hi << 8 | c_lo << 16 | c_hi << 24  (tile-local, half-open)
@@ -331,7 +341,9 @@ __global__ void __launch_bounds__(256, SHARP_OV_MINB) k_overlap(OverlapArgs A)
             for (int u = 0; u < UNR; ++u) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    if (!ok[u][k]) continue;
+                    // unconditional: a pair that is out of range was loaded as w = f = 0 and adds nothing.  (Predicating the
+                    // arithmetic as well keeps one of the 7 predicate registers live per pair from the load to its use, which
+                    // caps the loads ptxas can batch at 6-7 pairs.)
                     const float2 w_ = wa[u][k];
                     if constexpr (MODE == OV_DEN) {
                         dn[k] += w_.x * w_.x + w_.y * w_.y;
