@@ -35,6 +35,10 @@
 #include "fft_regs.cuh"
 #include "frame_common.cuh"
 
+#ifndef SHARP_S_PREFETCH
+#define SHARP_S_PREFETCH 1
+#endif
+
 namespace sharp {
 
 template <int M, int NT_>
@@ -358,7 +362,18 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
             }
             __syncwarp();
         }
-        cluster_barrier();
+        cluster_arrive();
+#if SHARP_S_PREFETCH
+        // between the arrive and the wait: pull the lines this CTA reads first in the cluster's NEXT frame (its stage-1
+        // column strips of the state) into L2, one stage ahead only (a whole frame ahead evicts the scratch, see above)
+        if (MODE == FRAME_ITER && i + nclusters < A.K) {
+            const float2 *nxt = A.c_in + (size_t)(i + nclusters) * M * M;
+            for (int s1 = crank; s1 < C::NSTR; s1 += CS)
+                for (int r = tid; r < M; r += NT)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(nxt + (size_t)r * M + s1 * WC));
+        }
+#endif
+        cluster_wait();
 
         // ---------------- stage 3: column strips ------------------------------------------------------------
         if constexpr (MODE == FRAME_ITER) {
