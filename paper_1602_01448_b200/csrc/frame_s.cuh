@@ -26,6 +26,8 @@
 // (m = 256: strips of 16 columns, four CTAs per SM) in clusters of 8: 929, in clusters of 4: 1212; the probe parked in
 // tensor memory (4 x 128 columns per SM): 1821 (the allocations of the four resident CTAs serialise), dropped.  Clusters
 // started in phases (what helps frame_r.cuh): 863 without, 863 / 869 with 8 phases of 2.5 / 5 us: no effect, dropped.
+// A per-line L2 prefetch of the CTA's next stage-1 strips, issued between the arrive and the wait of the second cluster
+// barrier (one stage ahead only): 861 against 863 at m = 256, 5.12 against 4.97 ms at config 5: dropped.
 // A bulk L2 prefetch of the cluster's next frame (what frame_r.cuh does) costs here: 926 with, 865 without (config 5:
 // 5.45 / 4.99 ms): the prefetched frames push the scratch frames out of L2.
 // The scratch frame (m^2 c64 per cluster) is the only data that leaves the SM between F and F*; it is re-used for
@@ -34,10 +36,6 @@
 #pragma once
 #include "fft_regs.cuh"
 #include "frame_common.cuh"
-
-#ifndef SHARP_S_PREFETCH
-#define SHARP_S_PREFETCH 1
-#endif
 
 namespace sharp {
 
@@ -363,16 +361,6 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
             __syncwarp();
         }
         cluster_arrive();
-#if SHARP_S_PREFETCH
-        // between the arrive and the wait: pull the lines this CTA reads first in the cluster's NEXT frame (its stage-1
-        // column strips of the state) into L2, one stage ahead only (a whole frame ahead evicts the scratch, see above)
-        if (MODE == FRAME_ITER && i + nclusters < A.K) {
-            const float2 *nxt = A.c_in + (size_t)(i + nclusters) * M * M;
-            for (int s1 = crank; s1 < C::NSTR; s1 += CS)
-                for (int r = tid; r < M; r += NT)
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(nxt + (size_t)r * M + s1 * WC));
-        }
-#endif
         cluster_wait();
 
         // ---------------- stage 3: column strips ------------------------------------------------------------
