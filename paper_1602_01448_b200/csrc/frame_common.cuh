@@ -135,29 +135,41 @@ __device__ __forceinline__ float frame_err_a32(const float2 *v, const float *ap,
     return sa;
 }
 
-// |P_Q z - z|^2 and |z - z_prev|^2 over a thread's 32 frame pixels (rows r_lo + NLO k of column col); v[] holds z
+// |P_Q z - z|^2 and |z - z_prev|^2 over a thread's 32 frame pixels (rows r_lo + NLO k of column col); v[] holds z.
+// Four pixels at a time: all loads of a batch are issued before its arithmetic (up to 20 per batch; eight spill), and the cases
+// (no previous iterate / previous iterate without an object part) are decided outside the loops.
 template <int M, int NLO>
 __device__ __forceinline__ void frame_err_qd32(const FrameArgs &A, const float2 *v, size_t fbase, int xr, int xc, int r_lo, int col,
                                                 float &sq, float &sd)
 {
     sq = 0.f;
     sd = 0.f;
+    int pcw = xc + col;                        // modulo the image size (identity without the periodic boundary)
+    if (pcw >= A.nc) pcw -= A.nc;
+    const bool have_prev = A.c_prev != nullptr, have_pv = have_prev && A.psi_v_prev != nullptr;
 #pragma unroll
-    for (int k = 0; k < 32; ++k) {
-        const int r = r_lo + NLO * k;
-        int prw = xr + r, pcw = xc + col;      // modulo the image size (identity without the periodic boundary)
-        if (prw >= A.nr) prw -= A.nr;
-        if (pcw >= A.nc) pcw -= A.nc;
-        const size_t op = (size_t)prw * A.nc + pcw;
-        const float2 d = csub(cmul(__ldg(A.w_cur + r * M + col), __ldg(A.psi_z + op)), v[k]);
-        sq += d.x * d.x + d.y * d.y;
-        float2 zp = make_float2(0.f, 0.f);
-        if (A.c_prev != nullptr) {
-            zp = ld_stream(A.c_prev + fbase + (size_t)r * M + col);
-            if (A.psi_v_prev != nullptr) zp = cadd(zp, cmul(__ldg(A.w_form_prev + r * M + col), __ldg(A.psi_v_prev + op)));
+    for (int k0 = 0; k0 < 32; k0 += 4) {
+        float2 wc[4], pz[4], cp[4], wp[4], pp[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int r = r_lo + NLO * (k0 + j);
+            int prw = xr + r;
+            if (prw >= A.nr) prw -= A.nr;
+            const size_t op = (size_t)prw * A.nc + pcw;
+            wc[j] = __ldg(A.w_cur + r * M + col);
+            pz[j] = __ldg(A.psi_z + op);
+            cp[j] = have_prev ? ld_stream(A.c_prev + fbase + (size_t)r * M + col) : make_float2(0.f, 0.f);
+            wp[j] = have_pv ? __ldg(A.w_form_prev + r * M + col) : make_float2(0.f, 0.f);
+            pp[j] = have_pv ? __ldg(A.psi_v_prev + op) : make_float2(0.f, 0.f);
         }
-        const float2 dd = csub(v[k], zp);
-        sd += dd.x * dd.x + dd.y * dd.y;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float2 d = csub(cmul(wc[j], pz[j]), v[k0 + j]);
+            sq += d.x * d.x + d.y * d.y;
+            const float2 zp = cadd(cp[j], cmul(wp[j], pp[j]));      // z_prev = c_prev + w_form_prev . T psi_v_prev (0 if absent)
+            const float2 dd = csub(v[k0 + j], zp);
+            sd += dd.x * dd.x + dd.y * dd.y;
+        }
     }
 }
 
