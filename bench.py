@@ -230,7 +230,7 @@ def measure(args, config_number, steps, warmup, rank, world, dev, dist, want_e2e
     cfg = synth.config(config_number)
     if args.grid:
         cfg = synth.reduced(cfg, args.grid)
-    sharded = bool(args.sharded) and world > 1
+    sharded = bool(args.sharded) and dist is not None
     if rank and not sharded:
         cfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
     iters = args.iters or cfg.iters
@@ -369,7 +369,9 @@ def run_ours(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     dist = None
-    if world > 1:
+    if world > 1 or (args.sharded and "RANK" in os.environ):
+        # (a one-rank group under torchrun --nproc-per-node 1 --sharded runs the sharded path through a real NCCL
+        # all-reduce: the only multi-GPU plumbing a one-GPU box can exercise)
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
@@ -423,7 +425,18 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
-    return run_ours(args)
+    # stdout carries the JSON line and nothing else: libraries that write banners to file descriptor 1 (NCCL prints its
+    # version there when NCCL_DEBUG=VERSION) are sent to stderr for the duration of the run
+    sys.stdout.flush()
+    saved = os.dup(1)
+    os.dup2(2, 1)
+    real_stdout = os.fdopen(saved, "w")
+    py_stdout, sys.stdout = sys.stdout, real_stdout
+    try:
+        return run_ours(args)
+    finally:
+        real_stdout.flush()
+        sys.stdout = py_stdout
 
 
 if __name__ == "__main__":

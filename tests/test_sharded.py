@@ -204,3 +204,45 @@ def test_sharded_reconstruction_matches_the_oracle(oracle, name, cfgno, grid, wo
         assert rel(r["w_init"], oracle.default_probe(I)) < 1e-5
         # all ranks hold the same object and illumination, bit for bit
         assert np.array_equal(r["psi"], results[0]["psi"]) and np.array_equal(r["w"], results[0]["w"])
+
+
+@pytest.mark.gpu
+def test_nccl_allreduce_callback_on_the_plan_stream(oracle):
+    """The real collective: a one-rank NCCL group (all this box has), `torch.distributed.all_reduce` handed to
+    sharp_set_sharded and called back by the library between its kernels on a non-default stream.  With one rank the sum is
+    the identity, so the run must reproduce the oracle; what is exercised is the C callback -> torch view of the workspace
+    -> NCCL launch ordered on the plan's stream, with no host synchronisation in between."""
+    import torch
+    import torch.distributed as dist
+    import paper_1602_01448_b200 as sharp
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(_free_port()))
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        cfg = synth.reduced(synth.config(3), 5)
+        pos, shape, I, w0, obj, wt = synth.make(cfg)
+        rng = np.random.default_rng(11)
+        z0 = (synth.exit_waves(cfg, obj, w0, pos) * (1 + 0.2 * (rng.standard_normal((cfg.K, cfg.m, cfg.m)) + 0j))).astype(np.complex64)
+        calls = []
+
+        def allreduce(t):
+            calls.append((t.dtype, t.numel()))
+            dist.all_reduce(t)
+
+        rec = sharp.Reconstruction(cfg.m, pos, shape, stream=torch.cuda.Stream())
+        rec.set_sharded(allreduce, cfg.K)
+        rec.set_intensities(I)
+        rec.set_probe(w0)
+        rec.set_probe_refine(1)
+        rec.set_frames(z0)
+        rec.iterate(3, cfg.beta)
+        z, eps, w = rec.get_frames().cpu().numpy(), rec.errors(), rec.get_probe().cpu().numpy()
+        rec.close()
+        o = oracle.Oracle(cfg.m, pos, shape, I, w0, refine_every=1)
+        o.set_frames(z0)
+        o.iterate(3, cfg.beta)
+        assert rel(z, o.z) < 5e-5 and rel(w, o.w) < 5e-5 and np.allclose(eps, o.errors(), rtol=1e-4)
+        nobj = shape[0] * shape[1]
+        assert (torch.float64, 1) in calls and (torch.float32, nobj) in calls and (torch.float32, 2 * nobj) in calls
+        assert (torch.float32, 3 * cfg.m * cfg.m) in calls and (torch.float64, 3) in calls
+    finally:
+        dist.destroy_process_group()
