@@ -48,6 +48,9 @@
 #ifndef SHARP_DYN
 #define SHARP_DYN 1
 #endif
+#ifndef SHARP_R_PIPE
+#define SHARP_R_PIPE 1
+#endif
 
 namespace sharp {
 
@@ -310,6 +313,21 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
     }
     __syncthreads();
 
+    // FRAME_ITER pipelines the state loads with the previous frame's stores: register v[k] is re-loaded with the next
+    // frame's value right after it has been stored (the loads enter the LSU queue between the stores instead of behind all
+    // of them), so the frame's own load of c happens only before a CTA's first frame.  Measured: 242.7 -> 241.2 us at
+    // config 2, 937 -> 900 us per 10,000 frames at config 6.
+    constexpr bool PIPE = (MODE == FRAME_ITER) && (SHARP_R_PIPE != 0);
+    float2 v[32];
+    if (PIPE) {
+        const int i0 = s_sched[0];
+        if (i0 < A.K) {
+            const float2 *cin = A.c_in + (size_t)i0 * M * M + (size_t)r_lo * M + col;
+#pragma unroll
+            for (int k = 0; k < 32; ++k) v[k] = ld_stream(cin + (size_t)k * (NLO * M));
+        }
+    }
+
     for (int par = 0;; par ^= 1) {
         const int i = s_sched[4 * par];
         if (i >= A.K) break;
@@ -328,13 +346,14 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
                 if (MODE != FRAME_FFT) prefetch_l2_bulk(A.a_int + (size_t)i_next * M * M, M * M * 4);
             }
         }
-        float2 v[32];
 
         // ---------------- P1: form z, DFT32 down the column -----------------------------------------------
         {
-            const float2 *cin = A.c_in + fbase + (size_t)r_lo * M + col;
+            if (!PIPE) {
+                const float2 *cin = A.c_in + fbase + (size_t)r_lo * M + col;
 #pragma unroll
-            for (int k = 0; k < 32; ++k) v[k] = ld_stream(cin + (size_t)k * (NLO * M));
+                for (int k = 0; k < 32; ++k) v[k] = ld_stream(cin + (size_t)k * (NLO * M));
+            }
             if (MODE == FRAME_FFT && A.conj_io) {
 #pragma unroll
                 for (int k = 0; k < 32; ++k) v[k].y = -v[k].y;
@@ -391,6 +410,7 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
             s_sched[4 * (par ^ 1) + 2] = nxc;
         }
         __syncthreads();                                                     // barrier 1
+        const int i_follow = PIPE ? s_sched[4 * (par ^ 1)] : 0;             // the frame after this one (uniform)
         // ---------------- P2: DFT32 along the row ----------------------------------------------------------
         P::p2_load(tid, E, v);
         dft<32, -1>(v);
@@ -444,8 +464,17 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
             P::p1_load(tid, E, v);
             dft<32, +1>(v);
             float2 *dst = A.c_out + fbase + (size_t)r_lo * M + col;
+            if (PIPE && i_follow < A.K) {
+                const float2 *cin = A.c_in + (size_t)i_follow * M * M + (size_t)r_lo * M + col;
 #pragma unroll
-            for (int k = 0; k < 32; ++k) st_stream(dst + (size_t)k * (NLO * M), v[k]);
+                for (int k = 0; k < 32; ++k) {
+                    st_stream(dst + (size_t)k * (NLO * M), v[k]);
+                    v[k] = ld_stream(cin + (size_t)k * (NLO * M));
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < 32; ++k) st_stream(dst + (size_t)k * (NLO * M), v[k]);
+            }
         }
     }
     if (w_tmem) {
