@@ -253,9 +253,12 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
     const float bm = A.bm, om = A.om;
     double s_a = 0.0, s_q = 0.0, s_d = 0.0;
 
-    // FRAME_ITER pipelines the loads of a frame's first stage-1 strip with the stores of the previous frame's last
-    // stage-3 strip (register v[k] is re-loaded right after it has been stored), as k_frame_r does: 866 -> 840 us at 1,600
-    // frames of 256 x 256, 4.95 -> 4.92 ms at config 5
+    // FRAME_ITER pipelines, at every strip transition, the loads of the next strip with the stores of the current one: register
+    // v[k] is re-loaded right after it has been stored, so the loads enter the LSU queue between the stores instead of behind
+    // all of them (stage 1: scratch stores / next strip's state; stage 2: scratch stores / next strip's scratch loads; stage 3:
+    // global stores / next strip's scratch loads, and for the last strip the first stage-1 strip of the cluster's next frame).
+    // Measured (us per launch at 1,600 frames of 256 x 256 / ms at config 5): none 866 / 4.95; frame transition only 840 / 4.92;
+    // all transitions 814 / 4.66.
     constexpr bool PIPE = (MODE == FRAME_ITER) && (SHARP_S_PIPE != 0);
     bool preloaded = false;
     float2 v[32];
@@ -267,7 +270,7 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
         for (int s1 = crank; s1 < C::NSTR; s1 += CS) {
             const int col = s1 * WC + col_l;
             {
-                if (!(PIPE && preloaded && s1 == crank)) {
+                if (!(PIPE && preloaded)) {
                     const float2 *cin = A.c_in + fbase + (size_t)r_lo * M + col;
 #pragma unroll
                     for (int k = 0; k < 32; ++k) v[k] = ld_stream(cin + (size_t)k * (NLO * M));
@@ -314,8 +317,19 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
             __syncthreads();
             P::p2_load(tid, E, v);
             P::template p2_math<false>(tid, tw, v);
+            preloaded = false;
+            if (PIPE && s1 + CS < C::NSTR) {     // the next strip's state is requested between this strip's scratch stores
+                const float2 *cin = A.c_in + fbase + (size_t)r_lo * M + (s1 + CS) * WC + col_l;
 #pragma unroll
-            for (int rho = 0; rho < 32; ++rho) s_st_scratch(scr + P::p2_scratch(tid, s1, rho), v[rho], pol_keep);
+                for (int rho = 0; rho < 32; ++rho) {
+                    s_st_scratch(scr + P::p2_scratch(tid, s1, rho), v[rho], pol_keep);
+                    v[rho] = ld_stream(cin + (size_t)rho * (NLO * M));
+                }
+                preloaded = true;
+            } else {
+#pragma unroll
+                for (int rho = 0; rho < 32; ++rho) s_st_scratch(scr + P::p2_scratch(tid, s1, rho), v[rho], pol_keep);
+            }
         }
         // this thread's 32 amplitudes of a row strip are requested well ahead of the projection: for the first strip
         // between the arrive and the wait of the cluster barrier, for the others before the forward transform
@@ -333,8 +347,11 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
 
         // ---------------- stage 2: row strips ---------------------------------------------------------------
         for (int s2 = crank; s2 < C::NSTR; s2 += CS) {
+            if (!(PIPE && preloaded)) {
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = s_ld_scratch(scr + P::p3_scratch(tid, s2, j), pol_keep);
+                for (int j = 0; j < 32; ++j) v[j] = s_ld_scratch(scr + P::p3_scratch(tid, s2, j), pol_keep);
+            }
+            preloaded = false;
             if (s2 != crank) load_amplitudes(s2);
             dft<32, -1>(v);
             __syncwarp();
@@ -365,8 +382,17 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
                     __syncwarp();
                     P::x3_load_cols(tid, E, v);
                     dft<32, +1>(v);
+                    if (PIPE && s2 + CS < C::NSTR) {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) s_st_scratch(scr + P::p3_scratch(tid, s2, j), v[j], pol_keep);
+                        for (int j = 0; j < 32; ++j) {
+                            s_st_scratch(scr + P::p3_scratch(tid, s2, j), v[j], pol_keep);
+                            v[j] = s_ld_scratch(scr + P::p3_scratch(tid, s2 + CS, j), pol_keep);
+                        }
+                        preloaded = true;
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) s_st_scratch(scr + P::p3_scratch(tid, s2, j), v[j], pol_keep);
+                    }
                 }
             }
             __syncwarp();
@@ -377,8 +403,11 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
         // ---------------- stage 3: column strips ------------------------------------------------------------
         if constexpr (MODE == FRAME_ITER) {
             for (int s1 = crank; s1 < C::NSTR; s1 += CS) {
+                if (!(PIPE && preloaded)) {
 #pragma unroll
-                for (int rho = 0; rho < 32; ++rho) v[rho] = s_ld_scratch(scr + P::p2_scratch(tid, s1, rho), pol_keep);
+                    for (int rho = 0; rho < 32; ++rho) v[rho] = s_ld_scratch(scr + P::p2_scratch(tid, s1, rho), pol_keep);
+                }
+                preloaded = false;
                 P::template p2_math<true>(tid, tw, v);
                 __syncthreads();             // the previous strip's X1 readers are done
                 P::p2_store(tid, E, v);
@@ -392,6 +421,13 @@ __global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
                     for (int k = 0; k < 32; ++k) {
                         st_stream(dst + (size_t)k * (NLO * M), v[k]);
                         v[k] = ld_stream(cin + (size_t)k * (NLO * M));
+                    }
+                    preloaded = true;
+                } else if (PIPE && s1 + CS < C::NSTR) {
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) {
+                        st_stream(dst + (size_t)k * (NLO * M), v[k]);
+                        v[k] = s_ld_scratch(scr + P::p2_scratch(tid, s1 + CS, k), pol_keep);
                     }
                     preloaded = true;
                 } else {
