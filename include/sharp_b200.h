@@ -215,6 +215,22 @@ int sharp_set_probe_recentre(sharp_plan_t *p, int on);
 int sharp_get_probe_shift(sharp_plan_t *p, int32_t last[2], int32_t total[2]);
 int sharp_op_probe_constrain(sharp_plan_t *p, const float *w_dev, float *out_dev);
 
+/* ---- allocation-free entry point --------------------------------------------------------------------------------
+ * sharp_fft2_noalloc: out_dev[K*m*m c64] <- F f (sign = -1) or F* f (sign = +1), unitary, natural order, DC at [0,0]
+ * (Eq. 2; the same kernel and the same results as sharp_op_fft2), for callers that cannot call
+ * cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it).  It needs no plan, no workspace and
+ * no sharp_bind: the kernel's transposition scratch lives in a static device array of the library (8 MiB + 32 KiB
+ * per GPU that loads the library, held until exit), and the call makes no cudaMalloc / cudaFree or other allocating call.
+ *   f_dev, out_dev   DEVICE, 16-byte aligned, distinct (out of place); the device that owns f_dev is used
+ *   m                256 only;  K in [1, SHARP_NOALLOC_MAX_FRAMES];  anything else: SHARP_EINVAL, text in
+ *                    sharp_last_error(NULL)
+ *   cuda_stream      cudaStream_t cast to void* (NULL = legacy default stream); asynchronous on it
+ * Every call shares the one static scratch: calls that overlap on the GPU (different streams without an ordering between
+ * them, or several host threads) race.  Calls on one stream are safe.  The scratch keeps the last call's contents;
+ * nothing in it has to start at zero (each frame's first stage writes every element before the second reads it). */
+#define SHARP_NOALLOC_MAX_FRAMES 4096
+int sharp_fft2_noalloc(const float *f_dev, float *out_dev, int m, int K, int sign, void *cuda_stream);
+
 /* ---- host-buffer convenience (the end-to-end path bench.py times) -----------------------------------------
  * sharp_reconstruct_host: everything from HOST buffers: uploads I (K*m*m f32) and w (m*m c64), runs n
  * iterations from the flat object, downloads psi (obj c64) and w, returns the three residuals.  The plan must

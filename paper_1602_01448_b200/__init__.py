@@ -61,6 +61,7 @@ _SIGNATURES = {
     "sharp_set_probe_recentre": (_i, [_vp, _i]),
     "sharp_get_probe_shift": (_i, [_vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]),
     "sharp_op_probe_constrain": (_i, [_vp, _vp, _vp]),
+    "sharp_fft2_noalloc": (_i, [_vp, _vp, _i, _i, _i, _vp]),
     "sharp_reconstruct_host": (_i, [_vp, _vp, _vp, _i, _f, _vp, _vp, C.POINTER(_f)]),
 }
 
@@ -94,6 +95,25 @@ def exported_symbols():
 
 def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(None)
+
+
+NOALLOC_MAX_FRAMES = 4096
+
+
+def fft2_noalloc(f, out, sign=-1, stream=None):
+    """sharp_fft2_noalloc: out <- F f (sign -1) / F* f (sign +1) for K frames of 256 x 256 complex64, with the kernel's
+    scratch in a static device array of the library (no plan, no workspace, no allocation inside the call).  `f` and `out`
+    are contiguous CUDA complex64 tensors of shape (K, 256, 256) allocated by the caller; asynchronous on `stream`
+    (default: torch's current stream).  Calls that overlap on the GPU share the scratch and race."""
+    import torch
+    lib = load_library()
+    assert f.is_cuda and out.is_cuda and f.dtype == out.dtype == torch.complex64 and f.is_contiguous() and out.is_contiguous()
+    assert f.shape == out.shape and f.dim() == 3
+    st = stream if stream is not None else torch.cuda.current_stream(f.device)
+    rc = lib.sharp_fft2_noalloc(_ptr(f), _ptr(out), int(f.shape[-1]), int(f.shape[0]), int(sign), C.c_void_p(st.cuda_stream))
+    if rc != SHARP_OK:
+        raise SharpError(rc, lib.sharp_last_error(None).decode())
+    return out
 
 
 class Reconstruction:

@@ -1230,3 +1230,90 @@ int sharp_op_probe_constrain(sharp_plan_t *p, const float *w_dev, float *out_dev
 }
 
 }  // extern "C"
+
+// ---- allocation-free entry point ------------------------------------------------------------------------------------
+// For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it): the batched
+// unitary 2-D DFT of 256 x 256 frames with the strip kernel's row<->column transposition scratch in a file-scope device
+// array instead of a caller workspace.  The arrays below are held by every GPU that loads the library until exit:
+//   g_noalloc_scratch   kNoAllocClusters (16) scratch frames of 256 x 256 c64 = 8 MiB
+//   g_noalloc_pos       positions the kernel reads per frame (unused by FRAME_FFT; stay zero), 32 KiB
+//   g_noalloc_scalars   DevScalars the kernel reads (unused by FRAME_FFT; stays zero)
+// In HOST code these names are host-side stand-ins, not device addresses: the addresses the kernel gets come from
+// cudaGetSymbolAddress, once per device, with that device current (noalloc_setup).  Nothing in the scratch has to start at
+// zero: stage 1 of every frame writes each scratch element before stage 2 reads it.  All calls share the arrays, so calls
+// that overlap on the GPU (different streams, no ordering between them) race.
+constexpr int kNoAllocM = 256;
+constexpr int kNoAllocClusters = 16;
+static_assert(SHARP_NOALLOC_MAX_FRAMES == 4096, "keep include/sharp_b200.h and the static arrays in step");
+static __device__ __align__(256) float2 g_noalloc_scratch[(size_t)kNoAllocClusters * kNoAllocM * kNoAllocM];
+static __device__ __align__(256) int g_noalloc_pos[2 * SHARP_NOALLOC_MAX_FRAMES];
+static __device__ __align__(256) DevScalars g_noalloc_scalars;
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+struct NoAllocDevice {
+    bool ready = false;
+    float2 *scratch = nullptr;
+    int *pos = nullptr;
+    DevScalars *scalars = nullptr;
+};
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+
+// once per device, with that device current: device addresses of the static arrays, shared-memory opt-in of the kernel
+int noalloc_setup(int dev, NoAllocDevice **out)
+{
+    sharp_plan_t *p = nullptr;      // CK reports through sharp_last_error(NULL)
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(nullptr, SHARP_EINVAL, "device ordinal %d not supported", dev);
+    NoAllocDevice &d = g_noalloc_dev[dev];
+    if (!d.ready) {
+        CK(cudaGetSymbolAddress((void **)&d.scratch, g_noalloc_scratch));
+        CK(cudaGetSymbolAddress((void **)&d.pos, g_noalloc_pos));
+        CK(cudaGetSymbolAddress((void **)&d.scalars, g_noalloc_scalars));
+        CK(cudaFuncSetAttribute(k_frame_s<256, kNT256, FRAME_FFT, kCluster256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                SCfg<256, kNT256>::SMEM_BYTES));
+        d.ready = true;
+    }
+    *out = &d;
+    return SHARP_OK;
+}
+
+}  // namespace
+
+extern "C" int sharp_fft2_noalloc(const float *f_dev, float *out_dev, int m, int K, int sign, void *cuda_stream)
+{
+    sharp_plan_t *p = nullptr;
+    if (!f_dev || !out_dev) return fail(nullptr, SHARP_EINVAL, "NULL argument");
+    if (f_dev == out_dev) return fail(nullptr, SHARP_EINVAL, "sharp_fft2_noalloc is out of place");
+    if (misaligned(f_dev) || misaligned(out_dev)) return fail(nullptr, SHARP_EINVAL, "device pointers must be 16-byte aligned");
+    if (m != kNoAllocM) return fail(nullptr, SHARP_EINVAL, "sharp_fft2_noalloc supports m = %d only (got %d)", kNoAllocM, m);
+    if (K < 1 || K > SHARP_NOALLOC_MAX_FRAMES)
+        return fail(nullptr, SHARP_EINVAL, "sharp_fft2_noalloc: K = %d outside [1, %d] (the static scratch is sized for that many frames)", K,
+                    SHARP_NOALLOC_MAX_FRAMES);
+    if (sign != 1 && sign != -1) return fail(nullptr, SHARP_EINVAL, "sign must be -1 (F) or +1 (F*)");
+    // run on the device that owns the input, whatever device is current
+    cudaPointerAttributes pa;
+    CK(cudaPointerGetAttributes(&pa, f_dev));
+    if (pa.type != cudaMemoryTypeDevice) return fail(nullptr, SHARP_EINVAL, "f_dev is not device memory");
+    int prev = -1;
+    CK(cudaGetDevice(&prev));
+    struct Restore { int d; ~Restore() { if (d >= 0) cudaSetDevice(d); } } restore{prev != pa.device ? prev : -1};
+    if (prev != pa.device) CK(cudaSetDevice(pa.device));
+    NoAllocDevice *d = nullptr;
+    if (int rc = noalloc_setup(pa.device, &d)) return rc;
+
+    FrameArgs a;
+    memset(&a, 0, sizeof a);
+    a.c_in = reinterpret_cast<const float2 *>(f_dev);
+    a.c_out = reinterpret_cast<float2 *>(out_dev);
+    a.scratch = d->scratch;          // the device address, NOT the symbol's host-side name
+    a.pos = d->pos;
+    a.sc = d->scalars;
+    a.K = K;
+    a.conj_io = (sign == 1);
+    const int clusters = std::min(K, kNoAllocClusters);
+    CK(launch_cluster(k_frame_s<256, kNT256, FRAME_FFT, kCluster256, false>, clusters * kCluster256, kNT256, SCfg<256, kNT256>::SMEM_BYTES,
+                      kCluster256, static_cast<cudaStream_t>(cuda_stream), a));
+    CK(cudaGetLastError());
+    return SHARP_OK;
+}
