@@ -51,6 +51,9 @@
 #ifndef SHARP_R_PIPE
 #define SHARP_R_PIPE 1
 #endif
+#ifndef SHARP_R_EARLY
+#define SHARP_R_EARLY 0
+#endif
 
 namespace sharp {
 
@@ -236,6 +239,19 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
     // P1 identity
     const int r_lo = wq % NLO, cblk = wq / NLO, col = 32 * cblk + lane;
 
+    // FRAME_ITER pipelines the state loads with the previous frame's stores: register v[k] is re-loaded with the next
+    // frame's value right after it has been stored (the loads enter the LSU queue between the stores instead of behind all
+    // of them), so the frame's own load of c happens only before a CTA's first frame.  Measured: 242.7 -> 241.2 us at
+    // config 2, 937 -> 900 us per 10,000 frames at config 6.  Issuing that first load before the twiddle / tensor-memory
+    // set-up and the start-up stagger (SHARP_R_EARLY) is slower, 244.3 against 241.4 us: all SMs then load in step again.
+    constexpr bool PIPE = (MODE == FRAME_ITER) && (SHARP_R_PIPE != 0);
+    float2 v[32];
+    if (PIPE && SHARP_R_EARLY && (int)blockIdx.x < A.K) {
+        const float2 *cin = A.c_in + (size_t)blockIdx.x * M * M + (size_t)r_lo * M + col;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) v[k] = ld_stream(cin + (size_t)k * (NLO * M));
+    }
+
     for (int k = tid; k < M; k += NT) {
         float sn, cs;
         sincospif(-2.0f * (float)k / (float)M, &sn, &cs);
@@ -313,13 +329,7 @@ __global__ void __launch_bounds__(RCfg<M>::NT, RCfg<M>::MIN_CTAS) k_frame_r(Fram
     }
     __syncthreads();
 
-    // FRAME_ITER pipelines the state loads with the previous frame's stores: register v[k] is re-loaded with the next
-    // frame's value right after it has been stored (the loads enter the LSU queue between the stores instead of behind all
-    // of them), so the frame's own load of c happens only before a CTA's first frame.  Measured: 242.7 -> 241.2 us at
-    // config 2, 937 -> 900 us per 10,000 frames at config 6.
-    constexpr bool PIPE = (MODE == FRAME_ITER) && (SHARP_R_PIPE != 0);
-    float2 v[32];
-    if (PIPE) {
+    if (PIPE && !SHARP_R_EARLY) {
         const int i0 = s_sched[0];
         if (i0 < A.K) {
             const float2 *cin = A.c_in + (size_t)i0 * M * M + (size_t)r_lo * M + col;
