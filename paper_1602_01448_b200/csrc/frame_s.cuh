@@ -26,6 +26,8 @@
 // (m = 256: strips of 16 columns, four CTAs per SM) in clusters of 8: 929, in clusters of 4: 1212; the probe parked in
 // tensor memory (4 x 128 columns per SM): 1821 (the allocations of the four resident CTAs serialise), dropped.  Clusters
 // started in phases (what helps frame_r.cuh): 863 without, 863 / 869 with 8 phases of 2.5 / 5 us: no effect, dropped.
+// Resident CTAs per SM at m = 256 (128 threads; registers per thread): 3 (168) 916 us, 4 (128, small spill) 814 us, 5 (96) 1051 us,
+// 6 (80) 1378 us; at m = 512 (256 threads) 2 (128) 4.66 ms, 3 (80) 8.60 ms.
 // A per-line L2 prefetch of the CTA's next stage-1 strips, issued between the arrive and the wait of the second cluster
 // barrier (one stage ahead only): 861 against 863 at m = 256, 5.12 against 4.97 ms at config 5: dropped.
 // A bulk L2 prefetch of the cluster's next frame (what frame_r.cuh does) costs here: 926 with, 865 without (config 5:
@@ -37,6 +39,9 @@
 #include "fft_regs.cuh"
 #include "frame_common.cuh"
 
+#ifndef SHARP_S_MINB
+#define SHARP_S_MINB(nt) (512 / (nt))
+#endif
 #ifndef SHARP_S_PIPE
 #define SHARP_S_PIPE 1
 #endif
@@ -225,7 +230,7 @@ __device__ __forceinline__ void s_st_scratch(float2 *p, float2 v, unsigned long 
 // Launched with cluster dimension CS; gridDim.x is a multiple of CS.  scratch: one m x m frame per cluster.
 // WRAP: periodic object index (see frame_r.cuh).
 template <int M, int NT_, int MODE, int CS, bool WRAP = false>
-__global__ void __launch_bounds__(NT_, 512 / NT_) k_frame_s(FrameArgs A)
+__global__ void __launch_bounds__(NT_, SHARP_S_MINB(NT_)) k_frame_s(FrameArgs A)
 {
     using C = SCfg<M, NT_>;
     using P = SPass<M, NT_>;
